@@ -1,0 +1,275 @@
+// api.cu -- the C ABI of include/bd.h: argument checking and stage sequencing only; every step of
+// the path runs in the kernels of assemble.cu / potrf.cu / brownian.cu / update.cu / observables.cu.
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "bd_internal.cuh"
+
+namespace {
+
+inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+
+bool layout_ok(const bd_ctx* ctx, const void* p, int64_t ld, int64_t stride)
+{
+    return p != nullptr && ld >= ctx->M && (ld % 2) == 0 && stride >= ld * (int64_t)ctx->M && (stride % 2) == 0 &&
+           (reinterpret_cast<uintptr_t>(p) % 16) == 0;
+}
+
+}  // namespace
+
+cudaError_t bd_g_last_cuda = cudaSuccess;
+
+extern "C" {
+
+int bd_create(const bd_params* params, void* cuda_stream, bd_ctx** out)
+{
+    if (params == nullptr) return -1;
+    if (out == nullptr) return -3;
+    *out = nullptr;
+    bd_params p = *params;
+    if (p.n_rods < 1 || p.n_chains < 1 || p.n_chains > 65535) return -1;
+    if (!(p.b > 0.0) || !(p.hstar >= 0.0) || !(p.dt > 0.0) || !std::isfinite(p.b) || !std::isfinite(p.hstar) || !std::isfinite(p.dt))
+        return -1;
+    if (!(p.a > 0.0)) p.a = p.hstar * p.b;                 // reading A3: a = h* b
+    if (p.hstar == 0.0 && !(p.a > 0.0)) p.a = p.b;         // free draining: a is irrelevant, keep it finite
+    if (p.hstar * p.b > p.a * (1.0 + 1e-12)) return -1;    // h*/a > 1: D not guaranteed positive definite (A3)
+    if (!(p.K > 0.0)) p.K = 1.0 / p.dt;                    // reading A6: K* dt = 1
+    if (p.noise_kind != 0 && p.noise_kind != 1) return -1;
+    for (int i = 0; i < 9; ++i)
+        if (!std::isfinite(p.kappa[i])) return -1;
+    if ((int64_t)3 * ((int64_t)p.n_rods + 1) > (int64_t)1 << 20) return -1;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        bd_g_last_cuda = cudaGetLastError();
+        return BD_ERR_CUDA;                               // no host fallback, by design
+    }
+    bd_ctx* ctx = new (std::nothrow) bd_ctx();
+    if (ctx == nullptr) return BD_ERR_ALLOC;
+    std::memset(ctx, 0, sizeof(*ctx));
+    ctx->p = p;
+    ctx->N = p.n_rods;
+    ctx->Nb = p.n_rods + 1;
+    ctx->M = 3 * ctx->Nb;
+    ctx->C = p.n_chains;
+    ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    ctx->ws_ld = round_up(ctx->M, 16);
+    ctx->ws_stride = ctx->ws_ld * (int64_t)ctx->M;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        bd_g_last_cuda = cudaGetLastError();
+        delete ctx;
+        return BD_ERR_CUDA;
+    }
+    ctx->num_sms = prop.multiProcessorCount;
+    const size_t CM = (size_t)ctx->C * ctx->M;
+    struct { void** p; size_t bytes; } allocs[] = {
+        {(void**)&ctx->T, sizeof(double) * (size_t)ctx->C * 3 * ctx->N},
+        {(void**)&ctx->F, sizeof(double) * CM},
+        {(void**)&ctx->v, sizeof(double) * CM},
+        {(void**)&ctx->y, sizeof(double) * CM},
+        {(void**)&ctx->dW, sizeof(double) * CM},
+        {(void**)&ctx->tmp, sizeof(double) * CM},
+        {(void**)&ctx->r_own, sizeof(double) * CM},
+        {(void**)&ctx->info, sizeof(int32_t) * (size_t)ctx->C},
+        {(void**)&ctx->fail, sizeof(int32_t) * 2},
+        {(void**)&ctx->obs, sizeof(double) * ((size_t)ctx->C + 2) * BD_NOBS},
+    };
+    for (auto& al : allocs) {
+        cudaError_t e = cudaMalloc(al.p, al.bytes);
+        if (e != cudaSuccess) {
+            bd_g_last_cuda = e;
+            bd_destroy(ctx);
+            return BD_ERR_CUDA;
+        }
+    }
+    cudaError_t e = cudaMemsetAsync(ctx->info, 0, sizeof(int32_t) * (size_t)ctx->C, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) {
+        bd_g_last_cuda = e;
+        bd_destroy(ctx);
+        return BD_ERR_CUDA;
+    }
+    *out = ctx;
+    return 0;
+}
+
+int bd_destroy(bd_ctx* ctx)
+{
+    if (ctx == nullptr) return -1;
+    cudaStreamSynchronize(ctx->stream);
+    void* ptrs[] = {ctx->T, ctx->F, ctx->v, ctx->y, ctx->dW, ctx->tmp, ctx->r_own, ctx->info, ctx->fail, ctx->obs};
+    for (void* q : ptrs)
+        if (q != nullptr) cudaFree(q);
+    delete ctx;
+    return 0;
+}
+
+size_t bd_workspace_bytes(const bd_ctx* ctx)
+{
+    if (ctx == nullptr) return 0;
+    return sizeof(double) * (size_t)ctx->C * (size_t)ctx->ws_stride;
+}
+
+int bd_set_workspace(bd_ctx* ctx, void* ws_dev, size_t bytes)
+{
+    if (ctx == nullptr) return -1;
+    if (ws_dev == nullptr || (reinterpret_cast<uintptr_t>(ws_dev) % 16) != 0) return -2;
+    if (bytes < bd_workspace_bytes(ctx)) return -3;
+    ctx->ws = static_cast<double*>(ws_dev);
+    ctx->ws_bytes = bytes;
+    return 0;
+}
+
+int bd_set_flow(bd_ctx* ctx, const double kappa_host[9])
+{
+    if (ctx == nullptr) return -1;
+    if (kappa_host == nullptr) return -2;
+    for (int i = 0; i < 9; ++i)
+        if (!std::isfinite(kappa_host[i])) return -2;
+    for (int i = 0; i < 9; ++i) ctx->p.kappa[i] = kappa_host[i];
+    return 0;
+}
+
+int bd_init_random_walk(bd_ctx* ctx, double* r_dev, uint64_t init_seed)
+{
+    if (ctx == nullptr) return -1;
+    if (r_dev == nullptr) return -2;
+    return bdk_init_random_walk(ctx, r_dev, init_seed);
+}
+
+int bd_assemble_hi(bd_ctx* ctx, const double* r_dev, double* D_dev, int64_t ld, int64_t chain_stride, int32_t full)
+{
+    if (ctx == nullptr) return -1;
+    if (r_dev == nullptr) return -2;
+    if (D_dev == nullptr || (reinterpret_cast<uintptr_t>(D_dev) % 16) != 0) return -3;
+    if (ld < ctx->M || (ld % 2) != 0) return -4;
+    if (chain_stride < ld * (int64_t)ctx->M || (chain_stride % 2) != 0) return -5;
+    return bdk_assemble(ctx, r_dev, D_dev, ld, chain_stride, full != 0);
+}
+
+int bd_cholesky(bd_ctx* ctx, double* DL_dev, int64_t ld, int64_t chain_stride, int32_t* info_dev)
+{
+    if (ctx == nullptr) return -1;
+    if (DL_dev == nullptr || (reinterpret_cast<uintptr_t>(DL_dev) % 16) != 0) return -2;
+    if (ld < ctx->M || (ld % 2) != 0) return -3;
+    if (chain_stride < ld * (int64_t)ctx->M || (chain_stride % 2) != 0) return -4;
+    int32_t* info = (info_dev != nullptr) ? info_dev : ctx->info;
+    BD_CUDA(ctx, cudaMemsetAsync(info, 0, sizeof(int32_t) * (size_t)ctx->C, ctx->stream));
+    return bdk_potrf(ctx, DL_dev, ld, chain_stride, info);
+}
+
+int bd_noise(bd_ctx* ctx, uint64_t step, double* dW_dev)
+{
+    if (ctx == nullptr) return -1;
+    if (dW_dev == nullptr) return -3;
+    return bdk_noise(ctx, step, dW_dev);
+}
+
+int bd_brownian(bd_ctx* ctx, const double* L_dev, int64_t ld, int64_t chain_stride, uint64_t step,
+                const double* dW_dev_or_null, double* y_dev)
+{
+    if (ctx == nullptr) return -1;
+    if (!layout_ok(ctx, L_dev, ld, chain_stride)) return (L_dev == nullptr) ? -2 : ((ld < ctx->M || ld % 2) ? -3 : -4);
+    if (y_dev == nullptr) return -7;
+    const double* dW = dW_dev_or_null;
+    if (dW == nullptr) {
+        int rc = bdk_noise(ctx, step, ctx->dW);
+        if (rc != 0) return rc;
+        dW = ctx->dW;
+    }
+    return bdk_trmv(ctx, L_dev, ld, chain_stride, dW, y_dev);
+}
+
+int bd_drift(bd_ctx* ctx, const double* r_dev, double* T_dev, double* F_dev, double* v_dev)
+{
+    if (ctx == nullptr) return -1;
+    if (r_dev == nullptr) return -2;
+    return bdk_drift(ctx, r_dev, T_dev, F_dev, v_dev);
+}
+
+int bd_update(bd_ctx* ctx, const double* r_dev, const double* v_dev, const double* y_dev, double* r_out_dev)
+{
+    if (ctx == nullptr) return -1;
+    if (r_dev == nullptr) return -2;
+    if (v_dev == nullptr) return -3;
+    if (y_dev == nullptr) return -4;
+    if (r_out_dev == nullptr) return -5;
+    return bdk_update(ctx, r_dev, v_dev, y_dev, nullptr, ctx->info, r_out_dev);
+}
+
+int bd_step(bd_ctx* ctx, double* r_dev, uint64_t first_step, int32_t n_steps)
+{
+    if (ctx == nullptr) return -1;
+    if (r_dev == nullptr) return -2;
+    if (n_steps < 0) return -4;
+    if (ctx->ws == nullptr) return BD_ERR_WORKSPACE;
+    BD_CUDA(ctx, cudaMemsetAsync(ctx->info, 0, sizeof(int32_t) * (size_t)ctx->C, ctx->stream));
+    for (int32_t s = 0; s < n_steps; ++s) {
+        int rc;
+        if ((rc = bdk_drift(ctx, r_dev, nullptr, ctx->F, ctx->v)) != 0) return rc;                       // a1, a4
+        if ((rc = bdk_assemble(ctx, r_dev, ctx->ws, ctx->ws_ld, ctx->ws_stride, 0)) != 0) return rc;     // a2
+        if ((rc = bdk_potrf(ctx, ctx->ws, ctx->ws_ld, ctx->ws_stride, ctx->info)) != 0) return rc;       // a3
+        if ((rc = bdk_noise(ctx, first_step + (uint64_t)s, ctx->dW)) != 0) return rc;                    // a0
+        if ((rc = bdk_trmv(ctx, ctx->ws, ctx->ws_ld, ctx->ws_stride, ctx->dW, ctx->y)) != 0) return rc;  // a5
+        if ((rc = bdk_update(ctx, r_dev, ctx->v, ctx->y, ctx->info, ctx->info, r_dev)) != 0) return rc;  // a6-a8
+    }
+    return 0;
+}
+
+int bd_observables(bd_ctx* ctx, const double* r_dev, double* per_chain_dev, double* ensemble_dev)
+{
+    if (ctx == nullptr) return -1;
+    if (r_dev == nullptr) return -2;
+    return bdk_observables(ctx, r_dev, per_chain_dev, ensemble_dev);
+}
+
+int bd_last_info(bd_ctx* ctx, int32_t* n_failed_chains, int32_t* first_failed_chain)
+{
+    if (ctx == nullptr) return -1;
+    int rc = bdk_count_failures(ctx, ctx->info);
+    if (rc != 0) return rc;
+    int32_t h[2] = {0, -1};
+    BD_CUDA(ctx, cudaMemcpyAsync(h, ctx->fail, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+    BD_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (n_failed_chains != nullptr) *n_failed_chains = h[0];
+    if (first_failed_chain != nullptr) *first_failed_chain = h[1];
+    return 0;
+}
+
+int bd_step_host(bd_ctx* ctx, double* r_host, uint64_t first_step, int32_t n_steps, double* ensemble_host)
+{
+    if (ctx == nullptr) return -1;
+    if (r_host == nullptr) return -2;
+    const size_t bytes = sizeof(double) * (size_t)ctx->C * ctx->M;
+    BD_CUDA(ctx, cudaMemcpyAsync(ctx->r_own, r_host, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    int rc = bd_step(ctx, ctx->r_own, first_step, n_steps);
+    if (rc != 0) return rc;
+    double* ens = ctx->obs + (size_t)ctx->C * BD_NOBS;
+    if ((rc = bdk_observables(ctx, ctx->r_own, ctx->obs, ens)) != 0) return rc;
+    BD_CUDA(ctx, cudaMemcpyAsync(r_host, ctx->r_own, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    if (ensemble_host != nullptr)
+        BD_CUDA(ctx, cudaMemcpyAsync(ensemble_host, ens, sizeof(double) * 2 * BD_NOBS, cudaMemcpyDeviceToHost, ctx->stream));
+    BD_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return 0;
+}
+
+int64_t bd_launch_count(const bd_ctx* ctx) { return (ctx == nullptr) ? 0 : ctx->launches; }
+
+const char* bd_strerror(int code)
+{
+    switch (code) {
+        case 0: return "success";
+        case BD_ERR_CUDA: return (bd_g_last_cuda != cudaSuccess) ? cudaGetErrorString(bd_g_last_cuda) : "CUDA runtime error (see cudaGetLastError)";
+        case BD_ERR_WORKSPACE: return "bd_step needs a workspace: call bd_set_workspace first";
+        case BD_ERR_ALLOC: return "host allocation failed";
+        default: break;
+    }
+    if (code < 0 && code > -20) return "invalid argument (index = -code)";
+    return "unknown error";
+}
+
+}  // extern "C"

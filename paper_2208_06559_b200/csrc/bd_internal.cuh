@@ -1,0 +1,104 @@
+// bd_internal.cuh -- context, launch helpers and small device utilities shared by the libbd kernels.
+// (Nothing here is shared with oracle/.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/bd.h"
+
+struct bd_ctx {
+    bd_params p;            // resolved parameters (a, K filled in)
+    int32_t N, Nb, M, C;
+    cudaStream_t stream;
+    int64_t ws_ld;          // leading dimension used by bd_step's own storage
+    int64_t ws_stride;      // doubles between chains in the workspace
+    double* ws;             // caller-owned D/L storage (bd_set_workspace)
+    size_t ws_bytes;
+    // O(C*M) scratch, library-owned
+    double* T;              // [C][N][3]
+    double* F;              // [C][Nb][3]
+    double* v;              // [C][M]
+    double* y;              // [C][M]
+    double* dW;             // [C][M]
+    double* Winv;           // [C][NB_INNER*NB_INNER] inverse of the current diagonal block
+    int32_t* info;          // [C]
+    int32_t* fail;          // [2]: count, first chain
+    double* obs;            // [C][BD_NOBS] + [2][BD_NOBS]
+    double* tmp;            // [C][M] unshifted positions inside the update / init kernels
+    double* r_own;          // [C][M] device positions for bd_step_host
+    int64_t launches;
+    cudaError_t last_cuda;
+    int num_sms;
+};
+
+extern cudaError_t bd_g_last_cuda;   // last CUDA error seen by any libbd call (for bd_strerror)
+
+#define BD_NB_INNER 64      // width of the diagonal block factored by potf2 (one CTA per chain)
+
+#define BD_CUDA(ctx, call)                                  \
+    do {                                                    \
+        cudaError_t e__ = (call);                           \
+        if (e__ != cudaSuccess) {                           \
+            (ctx)->last_cuda = e__;                         \
+            bd_g_last_cuda = e__;                           \
+            return BD_ERR_CUDA;                             \
+        }                                                   \
+    } while (0)
+
+// every kernel launch goes through this so that bd_launch_count is exact
+#define BD_LAUNCH(ctx, kernel, grid, block, smem, ...)                          \
+    do {                                                                        \
+        kernel<<<(grid), (block), (smem), (ctx)->stream>>>(__VA_ARGS__);        \
+        (ctx)->launches += 1;                                                   \
+        cudaError_t e__ = cudaGetLastError();                                   \
+        if (e__ != cudaSuccess) {                                               \
+            (ctx)->last_cuda = e__;                                             \
+            bd_g_last_cuda = e__;                                               \
+            return BD_ERR_CUDA;                                                 \
+        }                                                                       \
+    } while (0)
+
+// ---- stage entry points implemented in the .cu files (host side) -------------------------------
+int bdk_init_random_walk(bd_ctx* ctx, double* r, uint64_t init_seed);
+int bdk_assemble(bd_ctx* ctx, const double* r, double* D, int64_t ld, int64_t stride, int full);
+int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info);
+int bdk_noise(bd_ctx* ctx, uint64_t step, double* dW);
+int bdk_trmv(bd_ctx* ctx, const double* L, int64_t ld, int64_t stride, const double* dW, double* y);
+int bdk_drift(bd_ctx* ctx, const double* r, double* T, double* F, double* v);
+int bdk_update(bd_ctx* ctx, const double* r, const double* v, const double* y, const int32_t* info,
+               int32_t* info_out, double* r_out);
+int bdk_observables(bd_ctx* ctx, const double* r, double* per_chain, double* ensemble);
+int bdk_count_failures(bd_ctx* ctx, const int32_t* info);
+
+// ---- device helpers ------------------------------------------------------------------------------
+__device__ __forceinline__ double warp_sum(double x)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    return x;
+}
+__device__ __forceinline__ double warp_max(double x)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x = fmax(x, __shfl_xor_sync(0xffffffffu, x, o));
+    return x;
+}
+
+// RPY off-diagonal block coefficients (Eqs. 8-9): block = cI*I + cRR*Rv Rv^T with
+// Rv = (r_i - r_j)/b, a_s = a/b.  One rsqrt, no divisions: 1/R = rsqrt(R^2).
+__device__ __forceinline__ void rpy_coeffs(double R2, double hstar, double a_s, double& cI, double& cRR)
+{
+    if (R2 >= 4.0 * a_s * a_s) {                                   // Eq. 8, R >= 2a
+        double iR = rsqrt(R2);
+        double iR2 = iR * iR;
+        double pre = 0.75 * hstar * iR;
+        double a2 = a_s * a_s * iR2;
+        cI = pre * (1.0 + (2.0 / 3.0) * a2);
+        cRR = pre * (1.0 - 2.0 * a2) * iR2;
+    } else {                                                       // Eq. 9, R < 2a (finite at R -> 0)
+        double pre = 0.375 * hstar / a_s;
+        double iR = (R2 > 0.0) ? rsqrt(R2) : 0.0;
+        double R = R2 * iR;
+        cI = pre * (8.0 / 3.0 - 0.75 * R / a_s);
+        cRR = pre * 0.25 * iR / a_s;
+    }
+}

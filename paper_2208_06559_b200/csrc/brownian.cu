@@ -1,0 +1,83 @@
+// brownian.cu -- a0 (Brownian increments, Philox4x32-10 + Box-Muller) and a5 (y = L dW, the lower
+// triangular matvec of Eq. 6's third term).  HBM-read bound: 4 M^2 bytes per chain.
+#include "bd_internal.cuh"
+#include "philox.cuh"
+
+namespace {
+
+// one thread per pair p: dW[2p], dW[2p+1]
+__global__ void __launch_bounds__(256) k_noise(int M, uint64_t seed, uint64_t chain0, uint64_t step, int kind,
+                                               double dt, double* __restrict__ dW_all)
+{
+    const int c = blockIdx.y;
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (2 * p >= M) return;
+    double w0, w1;
+    brownian_pair(seed, (uint32_t)p, chain0 + (uint64_t)c, step, kind, dt, w0, w1);
+    double* dW = dW_all + (size_t)c * M;
+    dW[2 * p] = w0;
+    if (2 * p + 1 < M) dW[2 * p + 1] = w1;
+}
+
+// y_i = sum_{j<=i} L_ij dW_j.  One warp per row; lanes read 16-byte pairs, 4 independent loads in
+// flight per lane; rows are dealt to warps so that long and short rows mix inside a CTA.
+constexpr int kTrmvWarps = 8;
+
+__global__ void __launch_bounds__(kTrmvWarps * 32) k_trmv(int M, const double* __restrict__ L_all, int64_t ld, int64_t stride,
+                                                         const double* __restrict__ dW_all, double* __restrict__ y_all)
+{
+    const int c = blockIdx.y;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // pair short rows with long rows: CTA b takes rows b*4..b*4+3 from the top and the mirrored rows
+    const int nblk = gridDim.x;
+    const int half = nblk * (kTrmvWarps / 2);
+    int row;
+    if (warp < kTrmvWarps / 2) row = blockIdx.x * (kTrmvWarps / 2) + warp;
+    else row = 2 * half - 1 - (blockIdx.x * (kTrmvWarps / 2) + (warp - kTrmvWarps / 2));
+    if (row >= M) return;
+    const double* Lr = L_all + (size_t)c * stride + (size_t)row * ld;
+    const double* dW = dW_all + (size_t)c * M;
+    const int n = row + 1;                 // columns 0..row
+    const int n2 = n & ~1;
+    double acc0 = 0, acc1 = 0, acc2 = 0, acc3 = 0;
+    int j = 2 * lane;
+    for (; j + 192 < n2; j += 256) {
+        const double2 l0 = *reinterpret_cast<const double2*>(Lr + j);
+        const double2 l1 = *reinterpret_cast<const double2*>(Lr + j + 64);
+        const double2 l2 = *reinterpret_cast<const double2*>(Lr + j + 128);
+        const double2 l3 = *reinterpret_cast<const double2*>(Lr + j + 192);
+        // dW rows are only 8-byte aligned (M is odd): scalar loads, L1-resident
+        const double2 w0 = make_double2(dW[j], dW[j + 1]);
+        const double2 w1 = make_double2(dW[j + 64], dW[j + 65]);
+        const double2 w2 = make_double2(dW[j + 128], dW[j + 129]);
+        const double2 w3 = make_double2(dW[j + 192], dW[j + 193]);
+        acc0 += l0.x * w0.x + l0.y * w0.y;
+        acc1 += l1.x * w1.x + l1.y * w1.y;
+        acc2 += l2.x * w2.x + l2.y * w2.y;
+        acc3 += l3.x * w3.x + l3.y * w3.y;
+    }
+    for (; j < n2; j += 64) {
+        const double2 l0 = *reinterpret_cast<const double2*>(Lr + j);
+        acc0 += l0.x * dW[j] + l0.y * dW[j + 1];
+    }
+    if (lane == 0 && (n & 1)) acc1 += Lr[n - 1] * dW[n - 1];
+    const double s = warp_sum((acc0 + acc1) + (acc2 + acc3));
+    if (lane == 0) y_all[(size_t)c * M + row] = s;
+}
+
+}  // namespace
+
+int bdk_noise(bd_ctx* ctx, uint64_t step, double* dW)
+{
+    const int pairs = (ctx->M + 1) / 2;
+    BD_LAUNCH(ctx, k_noise, dim3((pairs + 255) / 256, ctx->C), dim3(256), 0, ctx->M, ctx->p.seed, ctx->p.chain_id0, step,
+              ctx->p.noise_kind, ctx->p.dt, dW);
+    return 0;
+}
+
+int bdk_trmv(bd_ctx* ctx, const double* L, int64_t ld, int64_t stride, const double* dW, double* y)
+{
+    const int nblk = (ctx->M + kTrmvWarps - 1) / kTrmvWarps;
+    BD_LAUNCH(ctx, k_trmv, dim3(nblk, ctx->C), dim3(kTrmvWarps * 32), 0, ctx->M, L, ld, stride, dW, y);
+    return 0;
+}

