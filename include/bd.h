@@ -129,6 +129,15 @@ int bd_last_info(bd_ctx *ctx, int32_t *n_failed_chains, int32_t *first_failed_ch
 int bd_step_host(bd_ctx *ctx, double *r_host, uint64_t first_step, int32_t n_steps,
                  double *ensemble_host);
 
+/* Stage timing for bench.py's roofline object.  bd_profile(ctx, 1) makes every later bd_step bracket
+ * its stages with CUDA events on the context's stream (first 1024 steps after enabling);
+ * bd_stage_ms synchronises, returns the accumulated milliseconds per stage
+ * [0 forces+drift a1/a4, 1 assemble a2, 2 cholesky a3, 3 noise a0, 4 L dW a5, 5 update a6-a8] and the
+ * number of steps they cover, and resets the accumulators.                                        */
+#define BD_NSTAGES 6
+int bd_profile(bd_ctx *ctx, int32_t enable);
+int bd_stage_ms(bd_ctx *ctx, double ms_host[BD_NSTAGES], int64_t *steps_host);
+
 /* Number of kernel launches issued through this context so far (for bench.py's gpu_launches).   */
 int64_t bd_launch_count(const bd_ctx *ctx);
 

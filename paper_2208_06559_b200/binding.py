@@ -28,8 +28,8 @@ class bd_params(C.Structure):
 
 EXPORTS = ("bd_create", "bd_destroy", "bd_workspace_bytes", "bd_set_workspace", "bd_set_flow",
            "bd_init_random_walk", "bd_assemble_hi", "bd_cholesky", "bd_brownian", "bd_noise", "bd_drift",
-           "bd_update", "bd_step", "bd_observables", "bd_last_info", "bd_step_host", "bd_launch_count",
-           "bd_strerror")
+           "bd_update", "bd_step", "bd_observables", "bd_last_info", "bd_step_host", "bd_profile",
+           "bd_stage_ms", "bd_launch_count", "bd_strerror")
 
 _lib = None
 
@@ -61,6 +61,8 @@ def load_library(path: str | None = None) -> C.CDLL:
     lib.bd_observables.argtypes = [vp, dp, dp, dp]
     lib.bd_last_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i32)]
     lib.bd_step_host.argtypes = [vp, dp, u64, i32, dp]
+    lib.bd_profile.argtypes = [vp, i32]
+    lib.bd_stage_ms.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
     lib.bd_launch_count.argtypes = [vp]
     lib.bd_launch_count.restype = i64
     lib.bd_strerror.argtypes = [C.c_int]
@@ -215,6 +217,18 @@ class BD:
         eh = C.c_void_p(ensemble_host.data_ptr()) if ensemble_host is not None else None
         self._check("bd_step_host", self.lib.bd_step_host(self._ctx, C.c_void_p(r_host.data_ptr()), first_step, n_steps, eh))
         return r_host
+
+    STAGES = ("drift", "assemble", "cholesky", "noise", "brownian", "update")
+
+    def profile(self, enable: bool = True):
+        self._check("bd_profile", self.lib.bd_profile(self._ctx, int(enable)))
+
+    def stage_ms(self):
+        """(dict stage -> accumulated ms, steps covered); synchronises and resets."""
+        ms = (C.c_double * 6)()
+        n = C.c_int64(0)
+        self._check("bd_stage_ms", self.lib.bd_stage_ms(self._ctx, ms, C.byref(n)))
+        return dict(zip(self.STAGES, [float(x) for x in ms])), int(n.value)
 
     def launch_count(self) -> int:
         return int(self.lib.bd_launch_count(self._ctx))

@@ -104,6 +104,11 @@ int bd_destroy(bd_ctx* ctx)
     void* ptrs[] = {ctx->T, ctx->F, ctx->v, ctx->y, ctx->dW, ctx->tmp, ctx->r_own, ctx->info, ctx->fail, ctx->obs};
     for (void* q : ptrs)
         if (q != nullptr) cudaFree(q);
+    if (ctx->ev != nullptr) {
+        for (int i = 0; i < ctx->ev_cap_steps * (BD_NSTAGES + 1); ++i)
+            if (ctx->ev[i] != nullptr) cudaEventDestroy(ctx->ev[i]);
+        std::free(ctx->ev);
+    }
     delete ctx;
     return 0;
 }
@@ -210,12 +215,23 @@ int bd_step(bd_ctx* ctx, double* r_dev, uint64_t first_step, int32_t n_steps)
     BD_CUDA(ctx, cudaMemsetAsync(ctx->info, 0, sizeof(int32_t) * (size_t)ctx->C, ctx->stream));
     for (int32_t s = 0; s < n_steps; ++s) {
         int rc;
+        cudaEvent_t* ev = nullptr;
+        if (ctx->prof_on && ctx->ev_steps < ctx->ev_cap_steps) ev = ctx->ev + (size_t)(ctx->ev_steps++) * (BD_NSTAGES + 1);
+#define BD_MARK(i) do { if (ev != nullptr) BD_CUDA(ctx, cudaEventRecord(ev[i], ctx->stream)); } while (0)
+        BD_MARK(0);
         if ((rc = bdk_drift(ctx, r_dev, nullptr, ctx->F, ctx->v)) != 0) return rc;                       // a1, a4
+        BD_MARK(1);
         if ((rc = bdk_assemble(ctx, r_dev, ctx->ws, ctx->ws_ld, ctx->ws_stride, 0)) != 0) return rc;     // a2
+        BD_MARK(2);
         if ((rc = bdk_potrf(ctx, ctx->ws, ctx->ws_ld, ctx->ws_stride, ctx->info)) != 0) return rc;       // a3
+        BD_MARK(3);
         if ((rc = bdk_noise(ctx, first_step + (uint64_t)s, ctx->dW)) != 0) return rc;                    // a0
+        BD_MARK(4);
         if ((rc = bdk_trmv(ctx, ctx->ws, ctx->ws_ld, ctx->ws_stride, ctx->dW, ctx->y)) != 0) return rc;  // a5
+        BD_MARK(5);
         if ((rc = bdk_update(ctx, r_dev, ctx->v, ctx->y, ctx->info, ctx->info, r_dev)) != 0) return rc;  // a6-a8
+        BD_MARK(6);
+#undef BD_MARK
     }
     return 0;
 }
@@ -254,6 +270,40 @@ int bd_step_host(bd_ctx* ctx, double* r_host, uint64_t first_step, int32_t n_ste
     if (ensemble_host != nullptr)
         BD_CUDA(ctx, cudaMemcpyAsync(ensemble_host, ens, sizeof(double) * 2 * BD_NOBS, cudaMemcpyDeviceToHost, ctx->stream));
     BD_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return 0;
+}
+
+int bd_profile(bd_ctx* ctx, int32_t enable)
+{
+    if (ctx == nullptr) return -1;
+    if (enable && ctx->ev == nullptr) {
+        const int cap = 1024;
+        ctx->ev = static_cast<cudaEvent_t*>(std::calloc((size_t)cap * (BD_NSTAGES + 1), sizeof(cudaEvent_t)));
+        if (ctx->ev == nullptr) return BD_ERR_ALLOC;
+        for (int i = 0; i < cap * (BD_NSTAGES + 1); ++i) BD_CUDA(ctx, cudaEventCreate(&ctx->ev[i]));
+        ctx->ev_cap_steps = cap;
+    }
+    ctx->prof_on = enable ? 1 : 0;
+    ctx->ev_steps = 0;
+    return 0;
+}
+
+int bd_stage_ms(bd_ctx* ctx, double ms_host[BD_NSTAGES], int64_t* steps_host)
+{
+    if (ctx == nullptr) return -1;
+    if (ms_host == nullptr) return -2;
+    BD_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int i = 0; i < BD_NSTAGES; ++i) ms_host[i] = 0.0;
+    for (int s = 0; s < ctx->ev_steps; ++s) {
+        cudaEvent_t* ev = ctx->ev + (size_t)s * (BD_NSTAGES + 1);
+        for (int i = 0; i < BD_NSTAGES; ++i) {
+            float ms = 0.f;
+            BD_CUDA(ctx, cudaEventElapsedTime(&ms, ev[i], ev[i + 1]));
+            ms_host[i] += (double)ms;
+        }
+    }
+    if (steps_host != nullptr) *steps_host = ctx->ev_steps;
+    ctx->ev_steps = 0;
     return 0;
 }
 

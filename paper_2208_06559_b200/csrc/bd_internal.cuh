@@ -26,6 +26,9 @@ struct bd_ctx {
     double* tmp;            // [C][M] unshifted positions inside the update / init kernels
     double* r_own;          // [C][M] device positions for bd_step_host
     int64_t launches;
+    // stage timing (bd_profile): (BD_NSTAGES+1) events per profiled step
+    cudaEvent_t* ev;
+    int32_t ev_cap_steps, ev_steps, prof_on;
     cudaError_t last_cuda;
     int num_sms;
 };
