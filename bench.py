@@ -127,6 +127,7 @@ def main():
     ap.add_argument("--config", default="c2", choices=sorted(W.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--path", type=int, default=0, help="bd_set_path: 0 auto, 1 staged kernels, 2 fused per-chain kernel")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     w = W.CONFIGS[args.config]
@@ -155,6 +156,7 @@ def main():
     bd = BD(n_rods=w.n_rods, n_chains=C, dt=w.dt, hstar=w.hstar, b=w.b, kappa=w.kappa(), seed=w.noise_seed,
             chain_id0=rank * C, device=f"cuda:{local_rank}")
     bd.set_workspace()
+    bd.set_path(args.path)
     r = bd.init_random_walk(w.init_seed)
     per, ens = bd.empty(C, NOBS), bd.empty(2, NOBS)
 
@@ -216,15 +218,20 @@ def main():
 
     if rank == 0:
         peaks = _peaks()
-        # dominant stage: the FP64 Cholesky (a dense contraction -> tensor roofline, FP64 DMMA peak)
-        chol_ms = stage["cholesky"] / max(nprof, 1)
+        # dominant kernel: the FP64 Cholesky (a dense contraction -> tensor roofline, FP64 DMMA peak).  On the fused
+        # short-chain path the whole step is ONE kernel (k_chain_step); its algorithmic flops are counted as the
+        # Cholesky flops only (M^3/3 + M^2/2 + M/6 per chain), the rest of the step is not credited.
+        fused = stage["fused"] > 0.0
+        chol_ms = (stage["fused"] if fused else stage["cholesky"]) / max(nprof, 1)
         chol_tflops = w.cholesky_flops() * C / (chol_ms * 1e-3) / 1e12 if chol_ms > 0 else None
         traffic = None
         try:
             traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(w.name)
         except Exception:
             pass
-        roofline = {"bound": "tensor", "kernel": "bd_cholesky stage (k_potf2 + k_trsm + k_syrk DMMA)",
+        roofline = {"bound": "tensor",
+                    "kernel": "k_chain_step<3> (fused a0-a8, one launch per step)" if fused else
+                              "bd_cholesky stage (k_potf2 + k_trsm + k_syrk DMMA)",
                     "achieved": chol_tflops, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                     "frac": (chol_tflops / FP64_PEAK_TFLOPS) if chol_tflops else None, "traffic": traffic,
                     "peak_source": "measured FP64 DMMA ceiling on B200 (148 SM x 64 FMA/clk x 1.957 GHz); "
@@ -243,9 +250,10 @@ def main():
                        "failed_chains": failed},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
             "stage_ms_per_step": stages,
-            "hbm_stages": {"assemble_GBps": (4.0 * w.M * w.M + 4.0 * w.M) * C / (asm_ms * 1e-3) / 1e9 if asm_ms > 0 else None,
-                           "brownian_GBps": 4.0 * w.M * w.M * C / (trmv_ms * 1e-3) / 1e9 if trmv_ms > 0 else None,
-                           "peak_GBps": hbm, "peak_source": "MEASURED_PEAKS.json" if peaks else "fallback"},
+            "hbm_stages": None if fused else {
+                "assemble_GBps": (4.0 * w.M * w.M + 4.0 * w.M) * C / (asm_ms * 1e-3) / 1e9 if asm_ms > 0 else None,
+                "brownian_GBps": 4.0 * w.M * w.M * C / (trmv_ms * 1e-3) / 1e9 if trmv_ms > 0 else None,
+                "peak_GBps": hbm, "peak_source": "MEASURED_PEAKS.json" if peaks else "fallback"},
             "cholesky_tflops": chol_tflops,
         }
         if world == 1 and not args.no_cpu_baseline:

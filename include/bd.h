@@ -68,7 +68,7 @@ typedef struct {
 int bd_create(const bd_params *params, void *cuda_stream, bd_ctx **out);
 int bd_destroy(bd_ctx *ctx);
 
-/* Bytes of matrix storage bd_step needs: C * M * ld * 8 with ld = M rounded up to 16.            */
+/* Bytes of matrix storage bd_step needs: C * ld * (M rounded up to 8) * 8, ld = M rounded up to 16. */
 size_t bd_workspace_bytes(const bd_ctx *ctx);
 /* Hand the context a caller-owned device buffer of at least bd_workspace_bytes (-2 if too small
  * or misaligned).  The buffer must outlive every later bd_step.                                  */
@@ -108,6 +108,12 @@ int bd_drift(bd_ctx *ctx, const double *r_dev, double *T_dev, double *F_dev, dou
 int bd_update(bd_ctx *ctx, const double *r_dev, const double *v_dev, const double *y_dev,
               double *r_out_dev);
 
+/* Which kernels bd_step uses.  0 (default): automatic -- the fused per-chain kernel (one persistent CTA
+ * per chain, D never stored, M <= 320) when the chain is short enough, else the staged kernels
+ * (assemble / blocked Cholesky / L dW / update) that the stage entry points above expose.
+ * 1: always staged.  2: always fused (-2 if M is too large).                                        */
+int bd_set_path(bd_ctx *ctx, int32_t path);
+
 /* The whole hot path a0-a8, n_steps times, time steps first_step .. first_step+n_steps-1;
  * r_dev [C][N_b][3] updated in place.  Needs bd_set_workspace.                                   */
 int bd_step(bd_ctx *ctx, double *r_dev, uint64_t first_step, int32_t n_steps);
@@ -132,9 +138,10 @@ int bd_step_host(bd_ctx *ctx, double *r_host, uint64_t first_step, int32_t n_ste
 /* Stage timing for bench.py's roofline object.  bd_profile(ctx, 1) makes every later bd_step bracket
  * its stages with CUDA events on the context's stream (first 1024 steps after enabling);
  * bd_stage_ms synchronises, returns the accumulated milliseconds per stage
- * [0 forces+drift a1/a4, 1 assemble a2, 2 cholesky a3, 3 noise a0, 4 L dW a5, 5 update a6-a8] and the
- * number of steps they cover, and resets the accumulators.                                        */
-#define BD_NSTAGES 6
+ * [0 forces+drift a1/a4, 1 assemble a2, 2 cholesky a3, 3 noise a0, 4 L dW a5, 5 update a6-a8,
+ * 6 the fused per-chain kernel (all of a0-a8) when that path is active] and the number of bd_step
+ * time steps they cover, and resets the accumulators.                                             */
+#define BD_NSTAGES 7
 int bd_profile(bd_ctx *ctx, int32_t enable);
 int bd_stage_ms(bd_ctx *ctx, double ms_host[BD_NSTAGES], int64_t *steps_host);
 

@@ -28,7 +28,7 @@ class bd_params(C.Structure):
 
 EXPORTS = ("bd_create", "bd_destroy", "bd_workspace_bytes", "bd_set_workspace", "bd_set_flow",
            "bd_init_random_walk", "bd_assemble_hi", "bd_cholesky", "bd_brownian", "bd_noise", "bd_drift",
-           "bd_update", "bd_step", "bd_observables", "bd_last_info", "bd_step_host", "bd_profile",
+           "bd_update", "bd_set_path", "bd_step", "bd_observables", "bd_last_info", "bd_step_host", "bd_profile",
            "bd_stage_ms", "bd_launch_count", "bd_strerror")
 
 _lib = None
@@ -57,6 +57,7 @@ def load_library(path: str | None = None) -> C.CDLL:
     lib.bd_noise.argtypes = [vp, u64, dp]
     lib.bd_drift.argtypes = [vp, dp, dp, dp, dp]
     lib.bd_update.argtypes = [vp, dp, dp, dp, dp]
+    lib.bd_set_path.argtypes = [vp, i32]
     lib.bd_step.argtypes = [vp, dp, u64, i32]
     lib.bd_observables.argtypes = [vp, dp, dp, dp]
     lib.bd_last_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i32)]
@@ -193,6 +194,10 @@ class BD:
         self._check("bd_update", self.lib.bd_update(self._ctx, _dptr(r), _dptr(v), _dptr(y), _dptr(r_out)))
         return r_out
 
+    def set_path(self, path: int):
+        """0 auto, 1 staged kernels, 2 fused per-chain kernel."""
+        self._check("bd_set_path", self.lib.bd_set_path(self._ctx, int(path)))
+
     def step(self, r, first_step: int = 0, n_steps: int = 1):
         if self._ws is None:
             self.set_workspace()
@@ -218,14 +223,14 @@ class BD:
         self._check("bd_step_host", self.lib.bd_step_host(self._ctx, C.c_void_p(r_host.data_ptr()), first_step, n_steps, eh))
         return r_host
 
-    STAGES = ("drift", "assemble", "cholesky", "noise", "brownian", "update")
+    STAGES = ("drift", "assemble", "cholesky", "noise", "brownian", "update", "fused")
 
     def profile(self, enable: bool = True):
         self._check("bd_profile", self.lib.bd_profile(self._ctx, int(enable)))
 
     def stage_ms(self):
         """(dict stage -> accumulated ms, steps covered); synchronises and resets."""
-        ms = (C.c_double * 6)()
+        ms = (C.c_double * 7)()
         n = C.c_int64(0)
         self._check("bd_stage_ms", self.lib.bd_stage_ms(self._ctx, ms, C.byref(n)))
         return dict(zip(self.STAGES, [float(x) for x in ms])), int(n.value)

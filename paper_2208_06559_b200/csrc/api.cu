@@ -56,7 +56,7 @@ int bd_create(const bd_params* params, void* cuda_stream, bd_ctx** out)
     ctx->C = p.n_chains;
     ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     ctx->ws_ld = round_up(ctx->M, 16);
-    ctx->ws_stride = ctx->ws_ld * (int64_t)ctx->M;
+    ctx->ws_stride = ctx->ws_ld * round_up(ctx->M, 8);
     int dev = 0;
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
@@ -108,6 +108,7 @@ int bd_destroy(bd_ctx* ctx)
         for (int i = 0; i < ctx->ev_cap_steps * (BD_NSTAGES + 1); ++i)
             if (ctx->ev[i] != nullptr) cudaEventDestroy(ctx->ev[i]);
         std::free(ctx->ev);
+        std::free(ctx->ev_nsteps);
     }
     delete ctx;
     return 0;
@@ -213,10 +214,27 @@ int bd_step(bd_ctx* ctx, double* r_dev, uint64_t first_step, int32_t n_steps)
     if (n_steps < 0) return -4;
     if (ctx->ws == nullptr) return BD_ERR_WORKSPACE;
     BD_CUDA(ctx, cudaMemsetAsync(ctx->info, 0, sizeof(int32_t) * (size_t)ctx->C, ctx->stream));
+    const bool fused = (ctx->path == 2) || (ctx->path == 0 && bdk_chain_step_supported(ctx));
+    if (fused) {
+        if (n_steps == 0) return 0;
+        cudaEvent_t* ev = nullptr;
+        if (ctx->prof_on && ctx->ev_steps < ctx->ev_cap_steps) {
+            ctx->ev_nsteps[ctx->ev_steps] = -n_steps;                       // negative: fused record
+            ev = ctx->ev + (size_t)(ctx->ev_steps++) * (BD_NSTAGES + 1);
+            BD_CUDA(ctx, cudaEventRecord(ev[0], ctx->stream));
+        }
+        int rc = bdk_chain_step(ctx, r_dev, first_step, n_steps);          // a0-a8, all steps, one launch
+        if (rc != 0) return rc;
+        if (ev != nullptr) BD_CUDA(ctx, cudaEventRecord(ev[1], ctx->stream));
+        return 0;
+    }
     for (int32_t s = 0; s < n_steps; ++s) {
         int rc;
         cudaEvent_t* ev = nullptr;
-        if (ctx->prof_on && ctx->ev_steps < ctx->ev_cap_steps) ev = ctx->ev + (size_t)(ctx->ev_steps++) * (BD_NSTAGES + 1);
+        if (ctx->prof_on && ctx->ev_steps < ctx->ev_cap_steps) {
+            ctx->ev_nsteps[ctx->ev_steps] = 1;
+            ev = ctx->ev + (size_t)(ctx->ev_steps++) * (BD_NSTAGES + 1);
+        }
 #define BD_MARK(i) do { if (ev != nullptr) BD_CUDA(ctx, cudaEventRecord(ev[i], ctx->stream)); } while (0)
         BD_MARK(0);
         if ((rc = bdk_drift(ctx, r_dev, nullptr, ctx->F, ctx->v)) != 0) return rc;                       // a1, a4
@@ -233,6 +251,15 @@ int bd_step(bd_ctx* ctx, double* r_dev, uint64_t first_step, int32_t n_steps)
         BD_MARK(6);
 #undef BD_MARK
     }
+    return 0;
+}
+
+int bd_set_path(bd_ctx* ctx, int32_t path)
+{
+    if (ctx == nullptr) return -1;
+    if (path < 0 || path > 2) return -2;
+    if (path == 2 && !bdk_chain_step_supported(ctx)) return -2;
+    ctx->path = path;
     return 0;
 }
 
@@ -281,6 +308,8 @@ int bd_profile(bd_ctx* ctx, int32_t enable)
         ctx->ev = static_cast<cudaEvent_t*>(std::calloc((size_t)cap * (BD_NSTAGES + 1), sizeof(cudaEvent_t)));
         if (ctx->ev == nullptr) return BD_ERR_ALLOC;
         for (int i = 0; i < cap * (BD_NSTAGES + 1); ++i) BD_CUDA(ctx, cudaEventCreate(&ctx->ev[i]));
+        ctx->ev_nsteps = static_cast<int32_t*>(std::calloc((size_t)cap, sizeof(int32_t)));
+        if (ctx->ev_nsteps == nullptr) return BD_ERR_ALLOC;
         ctx->ev_cap_steps = cap;
     }
     ctx->prof_on = enable ? 1 : 0;
@@ -294,15 +323,24 @@ int bd_stage_ms(bd_ctx* ctx, double ms_host[BD_NSTAGES], int64_t* steps_host)
     if (ms_host == nullptr) return -2;
     BD_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (int i = 0; i < BD_NSTAGES; ++i) ms_host[i] = 0.0;
+    int64_t nsteps = 0;
     for (int s = 0; s < ctx->ev_steps; ++s) {
         cudaEvent_t* ev = ctx->ev + (size_t)s * (BD_NSTAGES + 1);
-        for (int i = 0; i < BD_NSTAGES; ++i) {
+        if (ctx->ev_nsteps[s] < 0) {                                        // fused record: one interval
+            float ms = 0.f;
+            BD_CUDA(ctx, cudaEventElapsedTime(&ms, ev[0], ev[1]));
+            ms_host[BD_NSTAGES - 1] += (double)ms;
+            nsteps += -ctx->ev_nsteps[s];
+            continue;
+        }
+        for (int i = 0; i < BD_NSTAGES - 1; ++i) {
             float ms = 0.f;
             BD_CUDA(ctx, cudaEventElapsedTime(&ms, ev[i], ev[i + 1]));
             ms_host[i] += (double)ms;
         }
+        nsteps += 1;
     }
-    if (steps_host != nullptr) *steps_host = ctx->ev_steps;
+    if (steps_host != nullptr) *steps_host = nsteps;
     ctx->ev_steps = 0;
     return 0;
 }

@@ -16,7 +16,7 @@ constexpr int TROWS = 3 * TI;
 constexpr int TCOLS = 3 * TJ;
 constexpr int TLD = TCOLS + 2;        // padded smem row (keeps 16-byte alignment of pairs)
 
-__global__ void __launch_bounds__(TI * TJ) k_assemble(int Nb, double hstar, double a_s, double inv_b,
+__global__ void __launch_bounds__(TI * TJ) k_assemble(int Nb, double hstar, double a_s, double inv_a, double inv_b,
                                                       const double* __restrict__ r_all, double* __restrict__ D_all,
                                                       int64_t ld, int64_t stride, int full)
 {
@@ -39,7 +39,7 @@ __global__ void __launch_bounds__(TI * TJ) k_assemble(int Nb, double hstar, doub
         const double dx = (r[3 * i] - r[3 * j]) * inv_b, dy = (r[3 * i + 1] - r[3 * j + 1]) * inv_b,
                      dz = (r[3 * i + 2] - r[3 * j + 2]) * inv_b;
         double cI, cRR;
-        rpy_coeffs(dx * dx + dy * dy + dz * dz, hstar, a_s, cI, cRR);              // Eqs. 8-9
+        rpy_coeffs(dx * dx + dy * dy + dz * dz, hstar, a_s, inv_a, cI, cRR);              // Eqs. 8-9
         const double d[3] = {dx, dy, dz};
 #pragma unroll
         for (int k = 0; k < 3; ++k)
@@ -77,7 +77,7 @@ __global__ void __launch_bounds__(TI * TJ) k_assemble(int Nb, double hstar, doub
 int bdk_assemble(bd_ctx* ctx, const double* r, double* D, int64_t ld, int64_t stride, int full)
 {
     dim3 grid((ctx->Nb + TJ - 1) / TJ, (ctx->Nb + TI - 1) / TI, ctx->C);
-    BD_LAUNCH(ctx, k_assemble, grid, dim3(TI * TJ), 0, ctx->Nb, ctx->p.hstar, ctx->p.a / ctx->p.b, 1.0 / ctx->p.b, r, D, ld,
+    BD_LAUNCH(ctx, k_assemble, grid, dim3(TI * TJ), 0, ctx->Nb, ctx->p.hstar, ctx->p.a / ctx->p.b, ctx->p.b / ctx->p.a, 1.0 / ctx->p.b, r, D, ld,
               stride, full);
     return 0;
 }

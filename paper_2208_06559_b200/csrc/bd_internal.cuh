@@ -29,6 +29,8 @@ struct bd_ctx {
     // stage timing (bd_profile): (BD_NSTAGES+1) events per profiled step
     cudaEvent_t* ev;
     int32_t ev_cap_steps, ev_steps, prof_on;
+    int32_t* ev_nsteps;     // time steps covered by each profiled record
+    int32_t path;           // bd_set_path
     cudaError_t last_cuda;
     int num_sms;
 };
@@ -71,6 +73,8 @@ int bdk_update(bd_ctx* ctx, const double* r, const double* v, const double* y, c
                int32_t* info_out, double* r_out);
 int bdk_observables(bd_ctx* ctx, const double* r, double* per_chain, double* ensemble);
 int bdk_count_failures(bd_ctx* ctx, const int32_t* info);
+bool bdk_chain_step_supported(const bd_ctx* ctx);
+int bdk_chain_step(bd_ctx* ctx, double* r, uint64_t first_step, int n_steps);
 
 // ---- device helpers ------------------------------------------------------------------------------
 __device__ __forceinline__ double warp_sum(double x)
@@ -87,8 +91,8 @@ __device__ __forceinline__ double warp_max(double x)
 }
 
 // RPY off-diagonal block coefficients (Eqs. 8-9): block = cI*I + cRR*Rv Rv^T with
-// Rv = (r_i - r_j)/b, a_s = a/b.  One rsqrt, no divisions: 1/R = rsqrt(R^2).
-__device__ __forceinline__ void rpy_coeffs(double R2, double hstar, double a_s, double& cI, double& cRR)
+// Rv = (r_i - r_j)/b, a_s = a/b, inv_a = 1/a_s.  One rsqrt, no divisions: 1/R = rsqrt(R^2).
+__device__ __forceinline__ void rpy_coeffs(double R2, double hstar, double a_s, double inv_a, double& cI, double& cRR)
 {
     if (R2 >= 4.0 * a_s * a_s) {                                   // Eq. 8, R >= 2a
         double iR = rsqrt(R2);
@@ -98,10 +102,10 @@ __device__ __forceinline__ void rpy_coeffs(double R2, double hstar, double a_s, 
         cI = pre * (1.0 + (2.0 / 3.0) * a2);
         cRR = pre * (1.0 - 2.0 * a2) * iR2;
     } else {                                                       // Eq. 9, R < 2a (finite at R -> 0)
-        double pre = 0.375 * hstar / a_s;
+        double pre = 0.375 * hstar * inv_a;
         double iR = (R2 > 0.0) ? rsqrt(R2) : 0.0;
         double R = R2 * iR;
-        cI = pre * (8.0 / 3.0 - 0.75 * R / a_s);
-        cRR = pre * 0.25 * iR / a_s;
+        cI = pre * (8.0 / 3.0 - 0.75 * R * inv_a);
+        cRR = pre * 0.25 * iR * inv_a;
     }
 }

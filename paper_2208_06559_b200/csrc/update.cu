@@ -3,46 +3,11 @@
 // rebuild (a6-a8).  Citations: /root/reference/PAPER.md lines.
 #include "bd_internal.cuh"
 #include "philox.cuh"
+#include "block_ops.cuh"
 
 namespace {
 
 constexpr int kUpdThreads = 256;
-
-// Block-wide inclusive scan of three running sums over a chunk of blockDim.x items, plus carry-in.
-// s_warp: [3][32] scratch.  Returns the inclusive prefix for this thread; `carry` (per-thread copy of the
-// block-uniform running total) is advanced by the chunk total.
-__device__ __forceinline__ void block_scan3(double& x, double& y, double& z, double* s_warp, double carry[3])
-{
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        double tx = __shfl_up_sync(0xffffffffu, x, o);
-        double ty = __shfl_up_sync(0xffffffffu, y, o);
-        double tz = __shfl_up_sync(0xffffffffu, z, o);
-        if (lane >= o) { x += tx; y += ty; z += tz; }
-    }
-    __syncthreads();                       // protect s_warp from the previous chunk's readers
-    if (lane == 31) { s_warp[warp] = x; s_warp[32 + warp] = y; s_warp[64 + warp] = z; }
-    __syncthreads();
-    double ox = carry[0], oy = carry[1], oz = carry[2];
-    for (int w = 0; w < warp; ++w) { ox += s_warp[w]; oy += s_warp[32 + w]; oz += s_warp[64 + w]; }
-    x += ox; y += oy; z += oz;
-    double tx = 0, ty = 0, tz = 0;
-    for (int w = 0; w < nwarp; ++w) { tx += s_warp[w]; ty += s_warp[32 + w]; tz += s_warp[64 + w]; }
-    carry[0] += tx; carry[1] += ty; carry[2] += tz;
-}
-
-__device__ __forceinline__ double block_sum(double x, double* s_red)
-{
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
-    x = warp_sum(x);
-    __syncthreads();
-    if (lane == 0) s_red[warp] = x;
-    __syncthreads();
-    double t = 0;
-    for (int w = 0; w < nwarp; ++w) t += s_red[w];
-    return t;
-}
 
 // Rebuild positions from link vectors held one per thread per chunk: p_0 = 0, p_{k+1} = p_k + Q_k,
 // written unshifted to `tmp`, then shifted so that the centre of mass is 0 and written to r_out
@@ -129,7 +94,7 @@ __global__ void __launch_bounds__(256) k_forces(int N, double K, double b, const
 
 // a4: v_i = sum_j D_ij F_j (Eq. 6 second term, :102) with D_ij recomputed from positions (Eqs. 7-9),
 // so D is never read for the drift.  One warp per bead i, lanes stride over j.
-__global__ void __launch_bounds__(256) k_drift(int N, double hstar, double a_s, double inv_b,
+__global__ void __launch_bounds__(256) k_drift(int N, double hstar, double a_s, double inv_a, double inv_b,
                                                const double* __restrict__ r_all, const double* __restrict__ F_all,
                                                double* __restrict__ v_all)
 {
@@ -147,7 +112,7 @@ __global__ void __launch_bounds__(256) k_drift(int N, double hstar, double a_s, 
         if (j == i) { s0 += fx; s1 += fy; s2 += fz; continue; }          // Eq. 7: D_ii = I
         const double dx = (xi - r[3 * j]) * inv_b, dy = (yi - r[3 * j + 1]) * inv_b, dz = (zi - r[3 * j + 2]) * inv_b;
         double cI, cRR;
-        rpy_coeffs(dx * dx + dy * dy + dz * dz, hstar, a_s, cI, cRR);
+        rpy_coeffs(dx * dx + dy * dy + dz * dz, hstar, a_s, inv_a, cI, cRR);
         const double dot = cRR * (dx * fx + dy * fy + dz * fz);
         s0 += cI * fx + dot * dx; s1 += cI * fy + dot * dy; s2 += cI * fz + dot * dz;
     }
@@ -229,7 +194,7 @@ int bdk_drift(bd_ctx* ctx, const double* r, double* T, double* F, double* v)
         BD_LAUNCH(ctx, k_forces, dim3((ctx->Nb + 255) / 256, ctx->C), dim3(256), 0, ctx->N, ctx->p.K, ctx->p.b, r, T, Fbuf);
     if (v != nullptr)
         BD_LAUNCH(ctx, k_drift, dim3((ctx->Nb + 7) / 8, ctx->C), dim3(256), 0, ctx->N, ctx->p.hstar, ctx->p.a / ctx->p.b,
-                  1.0 / ctx->p.b, r, Fbuf, v);
+                  ctx->p.b / ctx->p.a, 1.0 / ctx->p.b, r, Fbuf, v);
     return 0;
 }
 

@@ -211,9 +211,10 @@ def test_update_matches_oracle(N, C):
 
 
 # ------------------------------------------------------------------------------------------ whole step
-def _step_parity(N, C, dt, hstar, kappa, steps, noise_kind=0, seed=0, jitter=0.007, rseed=0):
+def _step_parity(N, C, dt, hstar, kappa, steps, noise_kind=0, seed=0, jitter=0.007, rseed=0, path=0):
     r0 = W.random_chains(C, N, seed=rseed, rod_jitter=jitter)
     bd = _bd(N, C, dt, hstar=hstar, kappa=kappa, seed=seed, noise_kind=noise_kind)
+    bd.set_path(path)
     p = O.Params(n_rods=N, dt=dt, hstar=hstar, kappa=kappa if kappa is not None else np.zeros((3, 3)), seed=seed,
                  noise_kind=noise_kind)
     r = r0.copy()
@@ -229,23 +230,57 @@ def _step_parity(N, C, dt, hstar, kappa, steps, noise_kind=0, seed=0, jitter=0.0
     return worst_pos, worst_dr
 
 
+PATHS = [(1, "staged"), (2, "fused")]       # bd_set_path: staged kernels / fused per-chain kernel (M <= 320)
+FUSED_SIZES = [(1, 1), (2, 3), (7, 2), (8, 2), (15, 3), (20, 2), (21, 1), (42, 3), (100, 5), (105, 300)]
+
+
 @pytest.mark.parametrize("N,C", SIZES)
-def test_one_step_positions_match_oracle(N, C):
-    pos, dr = _step_parity(N, C, 1e-4, 0.25, KAPPA * 0.05, steps=2, rseed=N)
+def test_one_step_positions_match_oracle_staged(N, C):
+    pos, dr = _step_parity(N, C, 1e-4, 0.25, KAPPA * 0.05, steps=2, rseed=N, path=1)
     assert pos <= 1e-10                                          # BASELINE.json gate
     assert dr <= 1e-9                                            # the stricter displacement-relative figure (A16)
 
 
-def test_step_variants_uniform_noise_free_draining_shear():
-    assert _step_parity(30, 3, 1e-3, 0.5, None, steps=2, noise_kind=1, seed=77)[0] <= 1e-10   # paper's own law / h* = a* = 0.5
-    assert _step_parity(30, 3, 1e-4, 0.0, W.CONFIGS["c3"].kappa() * 100, steps=2)[0] <= 1e-10  # h* = 0, shear
-    assert _step_parity(64, 2, 5e-5, 0.25, W.CONFIGS["c2"].kappa(), steps=2)[0] <= 1e-10
+@pytest.mark.parametrize("N,C", FUSED_SIZES)
+def test_one_step_positions_match_oracle_fused(N, C):
+    """the fused per-chain kernel: ragged last panels (M % 24 != 0), one panel only (M <= 24), more chains
+    than resident CTAs (C = 300 > 2 x 148)."""
+    pos, dr = _step_parity(N, C, 1e-4, 0.25, KAPPA * 0.05, steps=2 if C < 100 else 1, rseed=N, path=2)
+    assert pos <= 1e-10
+    assert dr <= 1e-9
 
 
-def test_multi_step_call_equals_repeated_single_steps_and_tracks_oracle():
+@pytest.mark.parametrize("path,name", PATHS)
+def test_step_variants_uniform_noise_free_draining_shear(path, name):
+    assert _step_parity(30, 3, 1e-3, 0.5, None, steps=2, noise_kind=1, seed=77, path=path)[0] <= 1e-10   # paper's law, h* = a* = 0.5
+    assert _step_parity(30, 3, 1e-4, 0.0, W.CONFIGS["c3"].kappa() * 100, steps=2, path=path)[0] <= 1e-10  # h* = 0, shear
+    assert _step_parity(64, 2, 5e-5, 0.25, W.CONFIGS["c2"].kappa(), steps=2, path=path)[0] <= 1e-10
+
+
+def test_fused_and_staged_paths_agree():
+    N, C = 100, 16
+    r0 = W.random_chains(C, N, seed=31, rod_jitter=0.007)
+    outs = []
+    for path in (1, 2):
+        bd = _bd(N, C, 1e-4, kappa=W.CONFIGS["c2"].kappa(), seed=5)
+        bd.set_path(path)
+        outs.append(_host(bd.step(_dev(r0), 0, 3)))
+    assert np.abs(outs[0] - outs[1]).max() / np.abs(outs[0]).max() <= 1e-11
+
+
+def test_fused_path_rejected_for_long_chains():
+    from paper_2208_06559_b200.binding import BDError
+    bd = _bd(200, 1)
+    with pytest.raises(BDError):
+        bd.set_path(2)
+
+
+@pytest.mark.parametrize("path,name", PATHS)
+def test_multi_step_call_equals_repeated_single_steps_and_tracks_oracle(path, name):
     N, C, dt = 40, 4, 1e-4
     r0 = W.random_chains(C, N, seed=2)
     bd = _bd(N, C, dt, seed=11)
+    bd.set_path(path)
     a = _host(bd.step(_dev(r0), first_step=0, n_steps=6))
     rb = _dev(r0)
     for s in range(6):
@@ -255,11 +290,13 @@ def test_multi_step_call_equals_repeated_single_steps_and_tracks_oracle():
     assert np.abs(a - ro).max() / np.abs(ro).max() <= 1e-9       # free-running 6 steps: reported, loose
 
 
-def test_failed_chain_keeps_its_state():
+@pytest.mark.parametrize("path,name", PATHS)
+def test_failed_chain_keeps_its_state(path, name):
     N = 20
     r = W.random_chains(3, N, seed=9)
     r[1, 2] = r[1, 0]
     bd = _bd(N, 3)
+    bd.set_path(path)
     rg = _host(bd.step(_dev(r), 0, 1))
     assert np.array_equal(rg[1], r[1])                           # A10: reported, unchanged
     assert bd.last_info() == (1, 1)
