@@ -137,6 +137,7 @@ def main():
 
     import torch
     import torch.distributed as dist
+    from paper_2208_06559_b200 import ensemble
     from paper_2208_06559_b200.binding import BD, NOBS
 
     rank = int(os.environ.get("RANK", "0"))
@@ -154,7 +155,7 @@ def main():
 
     C, K = w.n_chains, args.steps
     bd = BD(n_rods=w.n_rods, n_chains=C, dt=w.dt, hstar=w.hstar, b=w.b, kappa=w.kappa(), seed=w.noise_seed,
-            chain_id0=rank * C, device=f"cuda:{local_rank}")
+            chain_id0=ensemble.shard(rank, world, C), device=f"cuda:{local_rank}")
     bd.set_workspace()
     bd.set_path(args.path)
     r = bd.init_random_walk(w.init_seed)
@@ -188,11 +189,8 @@ def main():
     stage, nprof = bd.stage_ms()
     bd.profile(False)
     clocks = sampler.stop() if rank == 0 else None
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-        dist.all_reduce(ens, op=dist.ReduceOp.SUM)          # the one exchange: ensemble accumulator (26 doubles)
+    ms = ensemble.max_over_ranks(ms, device="cuda")         # device-timed, max over ranks
+    ensemble.reduce_ensemble(ens)                           # the one exchange: ensemble accumulator (26 doubles)
     value = world * C * K / (ms * 1e-3)
     failed = bd.last_info()[0]
 
@@ -209,10 +207,7 @@ def main():
     e1.record()
     torch.cuda.synchronize(); barrier()
     ms_e2e = max(e0.elapsed_time(e1), 1e3 * (time.perf_counter() - t0))
-    if world > 1:
-        t = torch.tensor([ms_e2e], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
+    ms_e2e = ensemble.max_over_ranks(ms_e2e, device="cuda")
     e2e = {"value": world * C * K / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": C * w.M * 8,
            "d2h_bytes_per_step": C * w.M * 8 + 2 * NOBS * 8}
 
