@@ -77,6 +77,7 @@ int bd_create(const bd_params* params, void* cuda_stream, bd_ctx** out)
         {(void**)&ctx->info, sizeof(int32_t) * (size_t)ctx->C},
         {(void**)&ctx->fail, sizeof(int32_t) * 2},
         {(void**)&ctx->obs, sizeof(double) * ((size_t)ctx->C + 2) * BD_NOBS},
+        {(void**)&ctx->Winv, sizeof(double) * (size_t)ctx->C * BD_NB_INNER * BD_NB_INNER},
     };
     for (auto& al : allocs) {
         cudaError_t e = cudaMalloc(al.p, al.bytes);
@@ -101,7 +102,7 @@ int bd_destroy(bd_ctx* ctx)
 {
     if (ctx == nullptr) return -1;
     cudaStreamSynchronize(ctx->stream);
-    void* ptrs[] = {ctx->T, ctx->F, ctx->v, ctx->y, ctx->dW, ctx->tmp, ctx->r_own, ctx->info, ctx->fail, ctx->obs};
+    void* ptrs[] = {ctx->T, ctx->F, ctx->v, ctx->y, ctx->dW, ctx->tmp, ctx->r_own, ctx->info, ctx->fail, ctx->obs, ctx->Winv};
     for (void* q : ptrs)
         if (q != nullptr) cudaFree(q);
     if (ctx->ev != nullptr) {

@@ -17,6 +17,24 @@
 
 namespace {
 
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, int src_bytes)
+{
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(d), "l"(gsrc), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p)); }
+
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+
 // =================================================================================================
 // k_potf2: unblocked Cholesky of one nb x nb (nb <= 64) diagonal block per chain.  256 threads as a
 // 16 x 16 grid, thread (ty,tx) keeps the 4x4 sub-block rows 4ty.., cols 4tx.. in registers.  Step k
@@ -25,10 +43,11 @@ namespace {
 // A non-positive (or NaN) pivot d_k records info = 1-based global row (first failure wins).
 // =================================================================================================
 __global__ void __launch_bounds__(256) k_potf2(double* __restrict__ A_all, int64_t ld, int64_t stride, int j0, int nloc,
-                                               int32_t* __restrict__ info)
+                                               int32_t* __restrict__ info, double* __restrict__ Winv)
 {
     __shared__ double s_col[2][64];
     __shared__ double s_d[64];
+    __shared__ __align__(16) double s_Lt[64][66];   // s_Lt[j][i] = L[i][j] (column j of L contiguous in i), for the inverse
     const int c = blockIdx.x;
     double* A = A_all + (size_t)c * stride + (size_t)j0 * ld + j0;
     const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
@@ -87,185 +106,327 @@ __global__ void __launch_bounds__(256) k_potf2(double* __restrict__ A_all, int64
 #pragma unroll
             for (int rr = 0; rr < 4; ++rr) {
                 const int i = 4 * ty + rr;
-                if (i < nloc && j <= i) A[(size_t)i * ld + j] = (i == j) ? piv : a[rr][cc] * inv;
+                const double lv = (i == j) ? piv : a[rr][cc] * inv;
+                if (i < nloc && j <= i) A[(size_t)i * ld + j] = lv;
+                if (j <= i) s_Lt[j][i] = lv;
+            }
+        }
+    }
+    // W = L^-1 (lower), needed by the tensor-core triangular solve of the rows below (k_trsm): thread j
+    // forward-substitutes column j, right-looking so that every FMA of a step is independent; the
+    // column of L it needs at step i is a broadcast 16-byte shared-memory read.  Only full blocks
+    // have rows below them.
+    if (Winv == nullptr || nloc < 64) return;
+    __syncthreads();
+    if (threadIdx.x < 64) {
+        const int j = threadIdx.x;
+        double r[64];
+#pragma unroll
+        for (int i = 0; i < 64; ++i) r[i] = (i == j) ? 1.0 : 0.0;
+#pragma unroll
+        for (int i = 0; i < 64; ++i) {
+            const double wi = r[i] * rsqrt(s_d[i]);
+            r[i] = wi;
+            if (i & 1) {
+#pragma unroll
+                for (int m = i + 1; m < 64; m += 2) {
+                    const double2 l2 = *reinterpret_cast<const double2*>(&s_Lt[i][m]);
+                    r[m] -= l2.x * wi;
+                    r[m + 1] -= l2.y * wi;
+                }
+            } else {
+                r[i + 1] -= s_Lt[i][i + 1] * wi;
+#pragma unroll
+                for (int m = i + 2; m < 64; m += 2) {
+                    const double2 l2 = *reinterpret_cast<const double2*>(&s_Lt[i][m]);
+                    r[m] -= l2.x * wi;
+                    r[m + 1] -= l2.y * wi;
+                }
+            }
+        }
+        double* W = Winv + (size_t)c * 64 * 64;
+#pragma unroll
+        for (int i = 0; i < 64; ++i) W[i * 64 + j] = r[i];          // W[i][j], coalesced across the 64 threads
+    }
+}
+
+// =================================================================================================
+// k_trsm: rows gi in [r_lo, r_hi) of the panel at columns [j0, j0+64): X L^T = A  <=>  X = A W^T with
+// W = L^-1 (from k_potf2), i.e. X[r][c] = sum_{p <= c} A[r][p] W[c][p] -- a (rows x 64 x 64) product
+// on the FP64 tensor cores instead of a serial substitution per row.  One CTA = 128 rows; A tile and W
+// are staged once (cp.async) into shared memory with rows padded to 68 doubles (conflict-free 8-byte
+// fragment loads); 8 warps = 4 (32 rows) x 2 (column blocks nt = 2i + wn, interleaved so that the
+// triangular work 2(nt+1) k-steps per block balances); k-steps beyond the diagonal of W are skipped
+// with real branches.  In place: the tile is fully in shared memory before anything is written.
+// =================================================================================================
+constexpr int TRSM_ROWS = 128;
+constexpr int TRSM_SLD = 68;
+constexpr int TRSM_SMEM = (TRSM_ROWS + 64) * TRSM_SLD * (int)sizeof(double);
+
+template <int WN>
+__device__ __forceinline__ void trsm_warp(const double* __restrict__ a_base, const double* __restrict__ w_base, double (&acc)[4][4][2])
+{
+#pragma unroll
+    for (int ks = 0; ks < 16; ++ks) {
+        double af[4];
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt) af[mt] = a_base[mt * 8 * TRSM_SLD + ks * 4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            constexpr int dummy = 0; (void)dummy;
+            const int nt = 2 * i + WN;                       // columns 8nt .. 8nt+7 need p <= 8nt+7
+            if (4 * ks <= 8 * nt + 7) {
+                const double bf = w_base[nt * 8 * TRSM_SLD + ks * 4];
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt) dmma884(acc[mt][i][0], acc[mt][i][1], af[mt], bf);
             }
         }
     }
 }
 
-// =================================================================================================
-// k_trsm: rows gi in [r_lo, r_hi) of the panel at columns [j0, j0+64): solve X L^T = A in place with
-// the freshly factored 64x64 block L = A[j0.., j0..].  One thread per row (64 doubles in registers),
-// right-looking over the columns so that every FMA of a step is independent; L^T is broadcast from
-// shared memory with 16-byte loads.  Rows are staged through shared memory for coalesced global access.
-// =================================================================================================
-constexpr int TRSM_ROWS = 128;
-constexpr int TRSM_SLD = 65;          // odd stride: conflict-free row reads
-
-__global__ void __launch_bounds__(TRSM_ROWS) k_trsm(double* __restrict__ A_all, int64_t ld, int64_t stride, int j0,
-                                                    int r_lo, int r_hi)
+__global__ void __launch_bounds__(256, 2) k_trsm(double* __restrict__ A_all, int64_t ld, int64_t stride, int j0, int r_lo,
+                                                  int r_hi, const double* __restrict__ Winv)
 {
     extern __shared__ __align__(16) double smem[];
-    double* s_Lt = smem;                         // [64][64]  s_Lt[c][cp] = L[cp][c]  (column c of L, contiguous in cp)
-    double* s_inv = s_Lt + 64 * 64;              // [64]      1 / L[c][c]
-    double* s_X = s_inv + 64;                    // [TRSM_ROWS][TRSM_SLD]
+    double* sA = smem;                           // [128][68]
+    double* sW = smem + TRSM_ROWS * TRSM_SLD;    // [64][68]
     const int c = blockIdx.y;
     double* A = A_all + (size_t)c * stride;
+    const double* W = Winv + (size_t)c * 64 * 64;
     const int row0 = r_lo + blockIdx.x * TRSM_ROWS;
-    const int tid = threadIdx.x;
-    // L block (lower) -> transposed smem
-    for (int q = tid; q < 64 * 64; q += TRSM_ROWS) {
-        const int i = q >> 6, j = q & 63;
-        const double val = (j <= i) ? A[(size_t)(j0 + i) * ld + j0 + j] : 0.0;
-        s_Lt[j * 64 + i] = val;
-        if (i == j) s_inv[i] = 1.0 / val;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g = lane >> 2, t = lane & 3, wm = warp & 3, wn = warp >> 2;
+    {
+        const int lrow = tid >> 5, lch = tid & 31;           // 32 chunks of 16 bytes per 64-double row
+#pragma unroll
+        for (int it = 0; it < TRSM_ROWS / 8; ++it) {
+            const int rr = lrow + 8 * it;
+            const int gi = row0 + rr;
+            const bool ok = gi < r_hi;
+            cp_async16(sA + (size_t)rr * TRSM_SLD + 2 * lch, A + (size_t)(ok ? gi : r_hi - 1) * ld + j0 + 2 * lch, ok ? 16 : 0);
+        }
+#pragma unroll
+        for (int it = 0; it < 64 / 8; ++it) {
+            const int rr = lrow + 8 * it;
+            cp_async16(sW + (size_t)rr * TRSM_SLD + 2 * lch, W + (size_t)rr * 64 + 2 * lch, 16);
+        }
+        cp_async_commit();
+        cp_async_wait<0>();
+        __syncthreads();
     }
-    // panel rows -> smem (coalesced: 64 consecutive doubles per row)
-    for (int q = tid; q < TRSM_ROWS * 64; q += TRSM_ROWS) {
-        const int rr = q >> 6, cc = q & 63;
-        const int gi = row0 + rr;
-        s_X[rr * TRSM_SLD + cc] = (gi < r_hi) ? A[(size_t)gi * ld + j0 + cc] : 0.0;
-    }
-    __syncthreads();
-    double x[64];
+    double acc[4][4][2];
 #pragma unroll
-    for (int cc = 0; cc < 64; ++cc) x[cc] = s_X[tid * TRSM_SLD + cc];
+    for (int mt = 0; mt < 4; ++mt)
 #pragma unroll
-    for (int cc = 0; cc < 64; ++cc) {
-        const double xc = x[cc] * s_inv[cc];
-        x[cc] = xc;
-        const double* lt = s_Lt + cc * 64;
+        for (int i = 0; i < 4; ++i) acc[mt][i][0] = acc[mt][i][1] = 0.0;
+    const double* a_base = sA + (size_t)(wm * 32 + g) * TRSM_SLD + t;
+    const double* w_base = sW + (size_t)g * TRSM_SLD + t;
+    if (wn == 0) trsm_warp<0>(a_base, w_base, acc); else trsm_warp<1>(a_base, w_base, acc);
 #pragma unroll
-        for (int cp = cc + 1; cp < 64; ++cp) x[cp] -= xc * lt[cp];
-    }
+    for (int mt = 0; mt < 4; ++mt) {
+        const int gi = row0 + wm * 32 + mt * 8 + g;
+        if (gi >= r_hi) continue;
+        double* xrow = A + (size_t)gi * ld + j0;
 #pragma unroll
-    for (int cc = 0; cc < 64; ++cc) s_X[tid * TRSM_SLD + cc] = x[cc];
-    __syncthreads();
-    for (int q = tid; q < TRSM_ROWS * 64; q += TRSM_ROWS) {
-        const int rr = q >> 6, cc = q & 63;
-        const int gi = row0 + rr;
-        if (gi < r_hi) A[(size_t)gi * ld + j0 + cc] = s_X[rr * TRSM_SLD + cc];
+        for (int i = 0; i < 4; ++i) {
+            const int nt = 2 * i + wn;
+            *reinterpret_cast<double2*>(xrow + nt * 8 + 2 * t) = make_double2(acc[mt][i][0], acc[mt][i][1]);
+        }
     }
 }
 
 // =================================================================================================
-// k_syrk: for gi in [m_lo, m_hi), gj in [n_lo, n_hi), gj <= gi:
+// k_syrk: for gi in [lo, m_hi), gj in [lo, n_hi), gj <= gi:
 //     A[gi][gj] -= sum_{p in [k_lo, k_lo+K)} A[gi][p] * A[gj][p]
-// 128 x 128 tile per CTA, 8 warps (4 along m x 2 along n), warp tile 32 x 64 = 4 x 8 DMMA m8n8k4
-// accumulators (64 FP64 accumulators per thread).  Operands stream through a 4-stage cp.async
-// pipeline of 128 x 16 slabs; smem rows are padded to 20 doubles so the 8-byte fragment loads of a
-// warp fall in distinct bank pairs.
+// PERSISTENT: one CTA per SM walks the list of lower-triangular 128 x 128 tiles of all chains
+// (tile = blockIdx.x, + gridDim.x, ...).  8 warps (4 along m x 2 along n), warp tile 32 x 64 = 4 x 8
+// DMMA m8n8k4 accumulators (64 FP64 accumulators per thread).
+//   - C is loaded STRAIGHT INTO the accumulators (negated) when a tile starts and stored (negated back)
+//     when it ends: acc = -C + P P^T.  No load of C depends on anything in the epilogue, so the tensor
+//     pipe never waits on a DRAM round trip there (the first version's epilogue took 28 % of the
+//     kernel, profiles/r01_baseline_first_path.md); the next tile's C is prefetched into L2 meanwhile.
+//   - the operand pipeline (4-stage cp.async ring of 128 x 16 slabs) runs ACROSS tile boundaries: the
+//     load cursor is STAGES-1 k-slabs ahead of the compute cursor and simply moves on to the next tile.
+//   smem rows are padded to 20 doubles so the 8-byte fragment loads of a warp fall in distinct banks.
 // =================================================================================================
 constexpr int BM = 128, BN = 128, BK = 16, STAGES = 4, SLD = 20;
 constexpr int SYRK_SMEM = STAGES * (BM + BN) * SLD * (int)sizeof(double);
 
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, int src_bytes)
-{
-    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(d), "l"(gsrc), "r"(src_bytes));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+struct SyrkArgs {
+    double* A;
+    int64_t ld, stride;
+    int lo, m_hi, n_hi, k_lo, K;     // rows [lo, m_hi), columns [lo, n_hi), inner range [k_lo, k_lo+K)
+    int TN, tri, per_chain, total;   // tile columns, TN(TN+1)/2, tiles per chain, tiles in the launch
+};
 
-__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
+// tile index -> (chain, first row, first column).  Tiles (ty, tx), tx <= ty, tx < TN, row-major within a chain.
+__device__ __forceinline__ void syrk_tile(const SyrkArgs& a, int idx, int& chain, int& tm0, int& tn0)
 {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-                 : "+d"(c0), "+d"(c1)
-                 : "d"(a), "d"(b));
+    chain = idx / a.per_chain;
+    const int t = idx - chain * a.per_chain;
+    int ty, tx;
+    if (t < a.tri) {
+        ty = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
+        while ((ty + 1) * (ty + 2) / 2 <= t) ++ty;
+        while (ty * (ty + 1) / 2 > t) --ty;
+        tx = t - ty * (ty + 1) / 2;
+    } else {
+        const int u = t - a.tri;
+        ty = a.TN + u / a.TN;
+        tx = u - (u / a.TN) * a.TN;
+    }
+    tm0 = a.lo + ty * BM;
+    tn0 = a.lo + tx * BN;
 }
 
-__global__ void __launch_bounds__(256, 1) k_syrk(double* __restrict__ A_all, int64_t ld, int64_t stride, int m_lo, int m_hi,
-                                                 int n_lo, int n_hi, int k_lo, int K)
+__global__ void __launch_bounds__(256, 1) k_syrk(const SyrkArgs a)
 {
-    const int tm0 = m_lo + blockIdx.y * BM, tn0 = n_lo + blockIdx.x * BN;
-    if (tn0 > tm0 + BM - 1) return;                      // tile entirely above the diagonal
     extern __shared__ __align__(16) double smem[];
     double* sA = smem;                                   // [STAGES][BM][SLD]
     double* sB = smem + STAGES * BM * SLD;               // [STAGES][BN][SLD]
-    double* A = A_all + (size_t)blockIdx.z * stride;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm = warp & 3, wn = warp >> 2;
     const int g = lane >> 2, t = lane & 3;
-    const int KT = K / BK;
+    const int KT = a.K / BK;
+    const int64_t ld = a.ld;
 
-    auto load_stage = [&](int slot, int kt) {
-        const double* src_k = A + k_lo + kt * BK;
+    // ---- load cursor (runs STAGES-1 slabs ahead of the compute cursor) -----------------------------
+    int l_idx = blockIdx.x, l_kt = 0, l_tm0 = 0, l_tn0 = 0, l_chain = 0;
+    if (l_idx < a.total) syrk_tile(a, l_idx, l_chain, l_tm0, l_tn0);
+    const int lrow = tid >> 3, lch = tid & 7;            // this thread copies rows lrow, lrow+32, .. chunk lch
+    auto load_next = [&](int slot) {
+        if (l_idx < a.total) {
+            const double* src_k = a.A + (size_t)l_chain * a.stride + a.k_lo + l_kt * BK + 2 * lch;
+            double* dA = sA + ((size_t)slot * BM + lrow) * SLD + 2 * lch;
+            double* dB = sB + ((size_t)slot * BN + lrow) * SLD + 2 * lch;
 #pragma unroll
-        for (int it = 0; it < (BM * BK / 2) / 256; ++it) {
-            const int chunk = tid + it * 256;
-            const int row = chunk >> 3, ch = chunk & 7;
-            const int gr = tm0 + row;
-            const bool ok = gr < m_hi;
-            cp_async16(sA + ((size_t)slot * BM + row) * SLD + 2 * ch, src_k + (size_t)(ok ? gr : m_hi - 1) * ld + 2 * ch, ok ? 16 : 0);
-        }
+            for (int it = 0; it < BM / 32; ++it) {
+                const int gr = l_tm0 + lrow + 32 * it;
+                const bool ok = gr < a.m_hi;
+                cp_async16(dA + (size_t)it * 32 * SLD, src_k + (size_t)(ok ? gr : a.m_hi - 1) * ld, ok ? 16 : 0);
+            }
 #pragma unroll
-        for (int it = 0; it < (BN * BK / 2) / 256; ++it) {
-            const int chunk = tid + it * 256;
-            const int row = chunk >> 3, ch = chunk & 7;
-            const int gr = tn0 + row;
-            const bool ok = gr < n_hi;
-            cp_async16(sB + ((size_t)slot * BN + row) * SLD + 2 * ch, src_k + (size_t)(ok ? gr : n_hi - 1) * ld + 2 * ch, ok ? 16 : 0);
+            for (int it = 0; it < BN / 32; ++it) {
+                const int gr = l_tn0 + lrow + 32 * it;
+                const bool ok = gr < a.n_hi;
+                cp_async16(dB + (size_t)it * 32 * SLD, src_k + (size_t)(ok ? gr : a.n_hi - 1) * ld, ok ? 16 : 0);
+            }
+            if (++l_kt == KT) {
+                l_kt = 0;
+                l_idx += gridDim.x;
+                if (l_idx < a.total) syrk_tile(a, l_idx, l_chain, l_tm0, l_tn0);
+            }
         }
     };
 
-    double acc[4][8][2];
-#pragma unroll
-    for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-        for (int nt = 0; nt < 8; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
-
-    // this warp's 32 x 64 block lies entirely above the diagonal -> no arithmetic (still loads/syncs)
-    const bool warp_active = (tn0 + wn * 64) <= (tm0 + wm * 32 + 31);
-
 #pragma unroll
     for (int s = 0; s < STAGES - 1; ++s) {
-        if (s < KT) load_stage(s, s);
+        load_next(s);
         cp_async_commit();
     }
-    for (int kt = 0; kt < KT; ++kt) {
-        cp_async_wait<STAGES - 2>();
-        __syncthreads();
-        if (kt + STAGES - 1 < KT) load_stage((kt + STAGES - 1) % STAGES, kt + STAGES - 1);
-        cp_async_commit();
+
+    uint32_t git = 0;                                    // slabs consumed so far (ring position)
+    for (int idx = blockIdx.x; idx < a.total; idx += gridDim.x) {
+        int chain, tm0, tn0;
+        syrk_tile(a, idx, chain, tm0, tn0);
+        double* A = a.A + (size_t)chain * a.stride;
+        // this warp's 32 x 64 block lies entirely above the diagonal -> no arithmetic (still loads/syncs)
+        const bool warp_active = (tn0 + wn * 64) <= (tm0 + wm * 32 + 31);
+
+        // L2 prefetch of the NEXT tile's C (128 rows x 1 KB): its loads then cost an L2 hit, not a DRAM trip
+        if (idx + (int)gridDim.x < a.total) {
+            int nc, nm0, nn0;
+            syrk_tile(a, idx + gridDim.x, nc, nm0, nn0);
+            const double* Cn = a.A + (size_t)nc * a.stride;
+#pragma unroll
+            for (int it = 0; it < 4; ++it) {
+                const int q = tid + 256 * it;
+                const int gr = nm0 + (q >> 3), gc = nn0 + (q & 7) * 16;
+                if (gr < a.m_hi && gc <= gr && gc < a.n_hi) prefetch_l2(Cn + (size_t)gr * ld + gc);
+            }
+        }
+
+        double acc[4][8][2];
         if (warp_active) {
-            const double* a_base = sA + ((size_t)(kt % STAGES) * BM + wm * 32 + g) * SLD + t;
-            const double* b_base = sB + ((size_t)(kt % STAGES) * BN + wn * 64 + g) * SLD + t;
 #pragma unroll
-            for (int ks = 0; ks < BK / 4; ++ks) {
-                double af[4], bf[8];
+            for (int mt = 0; mt < 4; ++mt) {
+                const int gi = tm0 + wm * 32 + mt * 8 + g;
+                const double* crow = A + (size_t)gi * ld;
 #pragma unroll
-                for (int mt = 0; mt < 4; ++mt) af[mt] = a_base[mt * 8 * SLD + ks * 4];
+                for (int nt = 0; nt < 8; ++nt) {
+                    const int gj = tn0 + wn * 64 + nt * 8 + 2 * t;
+                    double c0 = 0.0, c1 = 0.0;
+                    if (gi < a.m_hi) {
+                        if (gj + 1 < a.n_hi && gj + 1 <= gi) {
+                            const double2 cv = *reinterpret_cast<const double2*>(crow + gj);
+                            c0 = cv.x; c1 = cv.y;
+                        } else if (gj < a.n_hi && gj <= gi) {
+                            c0 = crow[gj];
+                        }
+                    }
+                    acc[mt][nt][0] = -c0;
+                    acc[mt][nt][1] = -c1;
+                }
+            }
+        }
+
+        for (int kt = 0; kt < KT; ++kt, ++git) {
+            cp_async_wait<STAGES - 2>();
+            __syncthreads();
+            load_next((git + STAGES - 1) % STAGES);
+            cp_async_commit();
+            if (warp_active) {
+                const double* a_base = sA + ((size_t)(git % STAGES) * BM + wm * 32 + g) * SLD + t;
+                const double* b_base = sB + ((size_t)(git % STAGES) * BN + wn * 64 + g) * SLD + t;
 #pragma unroll
-                for (int nt = 0; nt < 8; ++nt) bf[nt] = b_base[nt * 8 * SLD + ks * 4];
+                for (int ks = 0; ks < BK / 4; ++ks) {
+                    double af[4], bf[8];
 #pragma unroll
-                for (int mt = 0; mt < 4; ++mt)
+                    for (int mt = 0; mt < 4; ++mt) af[mt] = a_base[mt * 8 * SLD + ks * 4];
 #pragma unroll
-                    for (int nt = 0; nt < 8; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], af[mt], bf[nt]);
+                    for (int nt = 0; nt < 8; ++nt) bf[nt] = b_base[nt * 8 * SLD + ks * 4];
+#pragma unroll
+                    for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                        for (int nt = 0; nt < 8; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], af[mt], bf[nt]);
+                }
+            }
+        }
+        if (warp_active) {
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt) {
+                const int gi = tm0 + wm * 32 + mt * 8 + g;
+                if (gi >= a.m_hi) continue;
+                double* crow = A + (size_t)gi * ld;
+#pragma unroll
+                for (int nt = 0; nt < 8; ++nt) {
+                    const int gj = tn0 + wn * 64 + nt * 8 + 2 * t;
+                    if (gj + 1 < a.n_hi && gj + 1 <= gi) {
+                        *reinterpret_cast<double2*>(crow + gj) = make_double2(-acc[mt][nt][0], -acc[mt][nt][1]);
+                    } else if (gj < a.n_hi && gj <= gi) {
+                        crow[gj] = -acc[mt][nt][0];
+                    }
+                }
             }
         }
     }
     cp_async_wait<0>();
-    if (!warp_active) return;
-    // epilogue: C -= acc on the lower triangle
-#pragma unroll
-    for (int mt = 0; mt < 4; ++mt) {
-        const int gi = tm0 + wm * 32 + mt * 8 + g;
-        if (gi >= m_hi) continue;
-        double* crow = A + (size_t)gi * ld;
-#pragma unroll
-        for (int nt = 0; nt < 8; ++nt) {
-            const int gj = tn0 + wn * 64 + nt * 8 + 2 * t;
-            if (gj + 1 < n_hi && gj + 1 <= gi) {
-                double2 cv = *reinterpret_cast<double2*>(crow + gj);
-                cv.x -= acc[mt][nt][0];
-                cv.y -= acc[mt][nt][1];
-                *reinterpret_cast<double2*>(crow + gj) = cv;
-            } else if (gj < n_hi && gj <= gi) {
-                crow[gj] -= acc[mt][nt][0];
-            }
-        }
-    }
+}
+
+// host side: rows [lo, m_hi) x columns [lo, n_hi) of every chain, inner range [k_lo, k_lo + K), K % 16 == 0
+int launch_syrk(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int lo, int m_hi, int n_hi, int k_lo, int K)
+{
+    SyrkArgs a;
+    a.A = A; a.ld = ld; a.stride = stride;
+    a.lo = lo; a.m_hi = m_hi; a.n_hi = n_hi; a.k_lo = k_lo; a.K = K;
+    const int TM = (m_hi - lo + BM - 1) / BM;
+    a.TN = (n_hi - lo + BN - 1) / BN;
+    a.tri = a.TN * (a.TN + 1) / 2;
+    a.per_chain = a.tri + (TM - a.TN) * a.TN;
+    a.total = a.per_chain * ctx->C;
+    const int grid = a.total < ctx->num_sms ? a.total : ctx->num_sms;
+    BD_LAUNCH(ctx, k_syrk, dim3(grid), dim3(256), SYRK_SMEM, a);
+    return 0;
 }
 
 }  // namespace
@@ -273,7 +434,7 @@ __global__ void __launch_bounds__(256, 1) k_syrk(double* __restrict__ A_all, int
 int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
 {
     static bool attr_set = false;
-    const int trsm_smem = (64 * 64 + 64 + TRSM_ROWS * TRSM_SLD) * (int)sizeof(double);
+    const int trsm_smem = TRSM_SMEM;
     if (!attr_set) {
         BD_CUDA(ctx, cudaFuncSetAttribute(k_syrk, cudaFuncAttributeMaxDynamicSharedMemorySize, SYRK_SMEM));
         BD_CUDA(ctx, cudaFuncSetAttribute(k_trsm, cudaFuncAttributeMaxDynamicSharedMemorySize, trsm_smem));
@@ -285,20 +446,20 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
         const int Jend = (J + NB < n) ? J + NB : n;
         for (int j = J; j < Jend; j += BD_NB_INNER) {
             const int nloc = (n - j < BD_NB_INNER) ? n - j : BD_NB_INNER;
-            BD_LAUNCH(ctx, k_potf2, dim3(C), dim3(256), 0, A, ld, stride, j, nloc, info);
+            BD_LAUNCH(ctx, k_potf2, dim3(C), dim3(256), 0, A, ld, stride, j, nloc, info, ctx->Winv);
             const int r_lo = j + BD_NB_INNER;
             if (r_lo < n) {
-                BD_LAUNCH(ctx, k_trsm, dim3((n - r_lo + TRSM_ROWS - 1) / TRSM_ROWS, C), dim3(TRSM_ROWS), trsm_smem, A, ld, stride, j,
-                          r_lo, n);
+                BD_LAUNCH(ctx, k_trsm, dim3((n - r_lo + TRSM_ROWS - 1) / TRSM_ROWS, C), dim3(256), trsm_smem, A, ld, stride, j,
+                          r_lo, n, ctx->Winv);
                 if (r_lo < Jend) {
-                    dim3 grid((Jend - r_lo + BN - 1) / BN, (n - r_lo + BM - 1) / BM, C);
-                    BD_LAUNCH(ctx, k_syrk, grid, dim3(256), SYRK_SMEM, A, ld, stride, r_lo, n, r_lo, Jend, j, BD_NB_INNER);
+                    int rc = launch_syrk(ctx, A, ld, stride, r_lo, n, Jend, j, BD_NB_INNER);
+                    if (rc != 0) return rc;
                 }
             }
         }
         if (Jend < n) {
-            dim3 grid((n - Jend + BN - 1) / BN, (n - Jend + BM - 1) / BM, C);
-            BD_LAUNCH(ctx, k_syrk, grid, dim3(256), SYRK_SMEM, A, ld, stride, Jend, n, Jend, n, J, Jend - J);
+            int rc = launch_syrk(ctx, A, ld, stride, Jend, n, n, J, Jend - J);
+            if (rc != 0) return rc;
         }
     }
     return 0;
