@@ -25,6 +25,7 @@
 #include "bd_internal.cuh"
 #include "block_ops.cuh"
 #include "philox.cuh"
+#include "warp_chol.cuh"
 
 namespace {
 
@@ -112,8 +113,6 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
 {
     constexpr int NBP = 8 * NT;            // panel width (columns)
     constexpr int NQP = NBP / 4;           // k-groups per panel
-    constexpr int G = NBP / 3;             // potf2 thread grid G x G, 3x3 elements per thread
-    constexpr int GT = ((G * G + 31) / 32) * 32;   // threads taking part in the pivot loop (whole warps)
     constexpr int PB = NBP / 3;            // beads per panel
     constexpr int WS = NBP + 4;            // row stride of W (conflict-free B fragments)
 
@@ -133,10 +132,8 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
     double* sV = sF + MP;                                       // [MP] drift D.F
     double* sY = sV + MP;                                       // [MP] L.dW
     double* sDW = sY + MP;                                      // [MP + NBP] Brownian increments, zero padded
-    double* sCol = sDW + MP + NBP;                              // [2][NBP]
-    double* sRow = sCol + 2 * NBP;                              // [2][NBP]
-    double* sD = sRow + 2 * NBP;                                // [NBP] pivots, then 1/sqrt(pivot)
-    double* sScan = sD + NBP;                                   // [96]
+    double* sCol = sDW + MP + NBP;                              // [2][32] column broadcast buffer of warp_chol_inv
+    double* sScan = sCol + 64;                                  // [96]
     __shared__ int sFail;
     __shared__ __align__(8) uint64_t sBar[2 * CS_STAGES];       // full[0..S), empty[S..2S)
 
@@ -189,22 +186,6 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
             for (int i = tid; i < MP; i += CS_THREADS) sY[i] = 0.0;
             if (tid == 0) sFail = 0;
             __syncthreads();
-            // ---- a4: drift v = D F, one warp per bead, D recomputed (Eqs. 7-9) -------------------------
-            for (int i = warp; i < Nb; i += CS_WARPS) {
-                const double xi = sR[3 * i], yi = sR[3 * i + 1], zi = sR[3 * i + 2];
-                double s0 = 0, s1 = 0, s2 = 0;
-                for (int j = lane; j < Nb; j += 32) {
-                    const double fx = sF[3 * j], fy = sF[3 * j + 1], fz = sF[3 * j + 2];
-                    if (j == i) { s0 += fx; s1 += fy; s2 += fz; continue; }
-                    const double dx = (xi - sR[3 * j]) * P.inv_b, dy = (yi - sR[3 * j + 1]) * P.inv_b, dz = (zi - sR[3 * j + 2]) * P.inv_b;
-                    double cI, cRR;
-                    rpy_coeffs(dx * dx + dy * dy + dz * dz, P.hstar, P.a_s, P.inv_a, cI, cRR);
-                    const double dot = cRR * (dx * fx + dy * fy + dz * fz);
-                    s0 += cI * fx + dot * dx; s1 += cI * fy + dot * dy; s2 += cI * fz + dot * dz;
-                }
-                s0 = warp_sum(s0); s1 = warp_sum(s1); s2 = warp_sum(s2);
-                if (lane == 0) { sV[3 * i] = s0; sV[3 * i + 1] = s1; sV[3 * i + 2] = s2; }
-            }
             CS_TIC(0);
 
             // ---- a2 + a3 + a5: left-looking blocked Cholesky with on-the-fly D and fused y = L dW ------
@@ -361,88 +342,47 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                 __syncthreads();
                 CS_TIC(3);
 
-                // (c) diagonal block: L_kk (in place in the tile) and W = L_kk^-1, G x G threads, 3x3 each.
-                //     Straight-line masked updates, shared-window addresses precomputed: the per-pivot
-                //     critical path is STS -> barrier -> LDS -> 1/d -> mul -> FMA.
-                if (tid < GT) {
-                    const int tx = tid % G, ty = tid / G;
-                    const bool in_grid = tid < G * G;
-                    const bool lower = in_grid && ty >= tx;
-                    double a[3][3], w[3][3];
+                // (c) diagonal block, warp 0: L_kk (back into the tile) and W = L_kk^-1 (-> winv), one row per lane,
+                //     registers + shuffles (warp_chol.cuh): ~100 cycles per pivot instead of a CTA barrier and a
+                //     division per pivot.  Warps 1..7 meanwhile compute this panel's slice of the drift v = D F
+                //     (a4, Eq. 6 second term; D blocks recomputed from positions, Eqs. 7-9), which nothing in the
+                //     factorisation depends on.
+                if (warp == 0) {
+                    double x[NBP];
 #pragma unroll
-                    for (int rr = 0; rr < 3; ++rr)
-#pragma unroll
-                        for (int cc = 0; cc < 3; ++cc) {
-                            const int i = 3 * ty + rr, j = 3 * tx + cc;
-                            double val = (i == j) ? 1.0 : 0.0;
-                            if (lower && i < pw && j <= i) val = tile[TIDX(i, j)];
-                            a[rr][cc] = val;
-                            w[rr][cc] = (i == j) ? 1.0 : 0.0;
-                        }
-                    const uint32_t col_u = smem_u32(sCol), row_u = smem_u32(sRow), d_u = smem_u32(sD);
-                    const uint32_t col_i = col_u + 8 * (3 * ty), col_j = col_u + 8 * (3 * tx), row_j = row_u + 8 * (3 * tx);
-                    CS_TIC(4);
-                    int kb = 0, kc = 0;
-                    for (int k = 0; k < pw; ++k) {
-                        const uint32_t buf = (uint32_t)(k & 1) * (8 * NBP);
-                        if (lower && tx == kb) {
-#pragma unroll
-                            for (int rr = 0; rr < 3; ++rr) sts_f64(col_i + buf + 8 * rr, (kc == 0) ? a[rr][0] : ((kc == 1) ? a[rr][1] : a[rr][2]));
-                        }
-                        if (lower && ty == kb) {
-#pragma unroll
-                            for (int cc = 0; cc < 3; ++cc) sts_f64(row_j + buf + 8 * cc, (kc == 0) ? w[0][cc] : ((kc == 1) ? w[1][cc] : w[2][cc]));
-                        }
-                        group_barrier(1, GT);
-                        const double d = lds_f64(col_u + buf + 8 * k);
-                        double ci[3], cj[3], rj[3];
-#pragma unroll
-                        for (int e = 0; e < 3; ++e) {
-                            ci[e] = lds_f64(col_i + buf + 8 * e);
-                            cj[e] = lds_f64(col_j + buf + 8 * e);
-                            rj[e] = lds_f64(row_j + buf + 8 * e);
-                        }
-                        if (tid == 0) {
-                            sts_f64(d_u + 8 * k, d);
-                            if (!(d > 0.0) && sFail == 0) sFail = k0 + k + 1;
-                        }
-                        const double invd = 1.0 / d;
-#pragma unroll
-                        for (int rr = 0; rr < 3; ++rr) {
-                            const double mi = (3 * ty + rr > k) ? ci[rr] * invd : 0.0;
-#pragma unroll
-                            for (int cc = 0; cc < 3; ++cc) {
-                                const bool right = 3 * tx + cc > k;
-                                a[rr][cc] -= mi * (right ? cj[cc] : 0.0);
-                                w[rr][cc] -= mi * (right ? 0.0 : rj[cc]);
-                            }
-                        }
-                        if (++kc == 3) { kc = 0; ++kb; }
+                    for (int j = 0; j < NBP; ++j) {
+                        double val = (lane == j) ? 1.0 : 0.0;                   // identity padding (ragged last panel)
+                        if (lane < pw && j < pw) val = tile[TIDX(max(lane, j), min(lane, j))];
+                        x[j] = (lane < NBP) ? val : 0.0;
                     }
-                    group_barrier(1, GT);
-                    CS_TIC(7);
-                    if (tid < NBP) sts_f64(d_u + 8 * tid, (tid < pw) ? rsqrt(lds_f64(d_u + 8 * tid)) : 1.0);     // 1/sqrt(d)
-                    group_barrier(1, GT);
-                    if (in_grid) {
+                    const bool row_ok = lane < NBP && k0 + lane < MP;
+                    const int f = warp_chol_inv<NBP, WS>(x, lane, sCol, winv, [&](int k, double l) {
+                        if (row_ok) tile[TIDX(lane, k)] = (lane >= k) ? l : 0.0;
+                    });
+                    __syncwarp();
+                    if (lane < NBP) {
 #pragma unroll
-                        for (int rr = 0; rr < 3; ++rr) {
-                            const int i = 3 * ty + rr;
-                            const double ri = sD[i];
-#pragma unroll
-                            for (int cc = 0; cc < 3; ++cc) {
-                                const int j = 3 * tx + cc;
-                                double lv = 0.0, wv = 0.0;
-                                if (j < i) {
-                                    lv = a[rr][cc] * sD[j];
-                                    wv = w[rr][cc] * ri;
-                                } else if (j == i) {
-                                    lv = (i < pw) ? 1.0 / ri : 1.0;          // sqrt(d) = 1 / (1/sqrt(d))
-                                    wv = ri;
-                                }
-                                if (k0 + i < MP) tile[TIDX(i, j)] = lv;
-                                winv[i * WS + j] = wv;
-                            }
+                        for (int c = 0; c < NBP; c += 2)
+                            *reinterpret_cast<double2*>(winv + lane * WS + c) = make_double2(x[c], x[c + 1]);
+                    }
+                    if (lane == 0 && f != 0 && sFail == 0) sFail = k0 + f;
+                } else {
+                    const int npan = (M + NBP - 1) / NBP, bps = (Nb + npan - 1) / npan;
+                    const int ib0 = (k0 / NBP) * bps, ib1 = min(ib0 + bps, Nb);
+                    for (int i = ib0 + warp - 1; i < ib1; i += CS_WARPS - 1) {
+                        const double xi = sR[3 * i], yi = sR[3 * i + 1], zi = sR[3 * i + 2];
+                        double s0 = 0, s1 = 0, s2 = 0;
+                        for (int j = lane; j < Nb; j += 32) {
+                            const double fx = sF[3 * j], fy = sF[3 * j + 1], fz = sF[3 * j + 2];
+                            if (j == i) { s0 += fx; s1 += fy; s2 += fz; continue; }
+                            const double dx = (xi - sR[3 * j]) * P.inv_b, dy = (yi - sR[3 * j + 1]) * P.inv_b, dz = (zi - sR[3 * j + 2]) * P.inv_b;
+                            double cI, cRR;
+                            rpy_coeffs(dx * dx + dy * dy + dz * dz, P.hstar, P.a_s, P.inv_a, cI, cRR);
+                            const double dot = cRR * (dx * fx + dy * fy + dz * fz);
+                            s0 += cI * fx + dot * dx; s1 += cI * fy + dot * dy; s2 += cI * fz + dot * dz;
                         }
+                        s0 = warp_sum(s0); s1 = warp_sum(s1); s2 = warp_sum(s2);
+                        if (lane == 0) { sV[3 * i] = s0; sV[3 * i + 1] = s1; sV[3 * i + 2] = s2; }
                     }
                 }
                 __syncthreads();
@@ -560,7 +500,7 @@ size_t chain_step_smem(int M)
     const int NBP = 8 * NT, MP = (M + 7) & ~7;
     const size_t slot_d = ((size_t)(MP - NBP > NBP ? MP - NBP : NBP) * 4 + 15) & ~(size_t)15;
     return sizeof(double) * (CS_STAGES * slot_d + (size_t)(NBP / 4) * (MP + 1) * 4 + (size_t)NBP * (NBP + 4) + 4 * (size_t)MP +
-                             (MP + NBP) + 5 * NBP + 96);
+                             (MP + NBP) + 64 + 96);
 }
 
 }  // namespace
