@@ -162,15 +162,15 @@ class BD:
         self._check("bd_init_random_walk", self.lib.bd_init_random_walk(self._ctx, _dptr(r), init_seed))
         return r
 
-    def assemble_hi(self, r, D=None, full: bool = False):
+    def assemble_hi(self, r, D=None, full: bool = False, chain_stride: int | None = None):
         D = self.matrix_storage() if D is None else D
         ld = D.shape[-1]
-        self._check("bd_assemble_hi", self.lib.bd_assemble_hi(self._ctx, _dptr(r), _dptr(D), ld, ld * self.M, int(full)))
+        self._check("bd_assemble_hi", self.lib.bd_assemble_hi(self._ctx, _dptr(r), _dptr(D), ld, chain_stride or ld * self.M, int(full)))
         return D
 
-    def cholesky(self, DL, info: torch.Tensor | None = None):
+    def cholesky(self, DL, info: torch.Tensor | None = None, chain_stride: int | None = None):
         ld = DL.shape[-1]
-        self._check("bd_cholesky", self.lib.bd_cholesky(self._ctx, _dptr(DL), ld, ld * self.M, _dptr(info)))
+        self._check("bd_cholesky", self.lib.bd_cholesky(self._ctx, _dptr(DL), ld, chain_stride or ld * self.M, _dptr(info)))
         return DL
 
     def noise(self, step: int, dW=None):
@@ -178,10 +178,10 @@ class BD:
         self._check("bd_noise", self.lib.bd_noise(self._ctx, step, _dptr(dW)))
         return dW
 
-    def brownian(self, L, step: int = 0, dW=None, y=None):
+    def brownian(self, L, step: int = 0, dW=None, y=None, chain_stride: int | None = None):
         y = self.empty(self.C, self.M) if y is None else y
         ld = L.shape[-1]
-        self._check("bd_brownian", self.lib.bd_brownian(self._ctx, _dptr(L), ld, ld * self.M, step, _dptr(dW), _dptr(y)))
+        self._check("bd_brownian", self.lib.bd_brownian(self._ctx, _dptr(L), ld, chain_stride or ld * self.M, step, _dptr(dW), _dptr(y)))
         return y
 
     def drift(self, r):

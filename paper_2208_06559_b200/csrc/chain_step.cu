@@ -417,6 +417,9 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
 #pragma unroll
                     for (int nt = 0; nt < NT; ++nt) {
                         part += x[nt][0] * sDW[k0 + 8 * nt + 2 * t] + x[nt][1] * sDW[k0 + 8 * nt + 2 * t + 1];
+                        // columns >= MP (ragged last panel) do not exist in Lg: k-group q >= MP/4 would land in the
+                        // NEXT CTA's scratch (rows 8mt.. of its k-groups 0, 1) and corrupt a chain in flight there
+                        if (k0 + 8 * nt >= MP) continue;
                         const int q = (k0 >> 2) + 2 * nt + (t >> 1);
                         *reinterpret_cast<double2*>(Lg + ((size_t)q * MP + 8 * mt + g) * 4 + 2 * (t & 1)) = make_double2(x[nt][0], x[nt][1]);
                     }
