@@ -132,8 +132,9 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
     double* sV = sF + MP;                                       // [MP] drift D.F
     double* sY = sV + MP;                                       // [MP] L.dW
     double* sDW = sY + MP;                                      // [MP + NBP] Brownian increments, zero padded
-    double* sCol = sDW + MP + NBP;                              // [2][32] column broadcast buffer of warp_chol_inv
+    double* sCol = sDW + MP + NBP;                              // [2][32] column broadcast buffer of warp_chol
     double* sScan = sCol + 64;                                  // [96]
+    double* sRinv = sScan + 96;                                 // [32] 1 / L_kk of the current diagonal block
     __shared__ int sFail;
     __shared__ __align__(8) uint64_t sBar[2 * CS_STAGES];       // full[0..S), empty[S..2S)
 
@@ -347,6 +348,7 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                 //     division per pivot.  Warps 1..7 meanwhile compute this panel's slice of the drift v = D F
                 //     (a4, Eq. 6 second term; D blocks recomputed from positions, Eqs. 7-9), which nothing in the
                 //     factorisation depends on.
+                const int nrows = min(NBP, MP - k0);                           // rows of the block that exist (ragged last panel)
                 if (warp == 0) {
                     double x[NBP];
 #pragma unroll
@@ -355,21 +357,19 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                         if (lane < pw && j < pw) val = tile[TIDX(max(lane, j), min(lane, j))];
                         x[j] = (lane < NBP) ? val : 0.0;
                     }
-                    const bool row_ok = lane < NBP && k0 + lane < MP;
-                    const int f = warp_chol_inv<NBP, WS>(x, lane, sCol, winv, [&](int k, double l) {
+                    const bool row_ok = lane < nrows;
+                    __syncwarp();
+                    const int f = warp_chol<NBP, 8>(x, lane, sCol, sRinv, 1, [&](int k, double l) {
                         if (row_ok) tile[TIDX(lane, k)] = (lane >= k) ? l : 0.0;
                     });
-                    __syncwarp();
-                    if (lane < NBP) {
-#pragma unroll
-                        for (int c = 0; c < NBP; c += 2)
-                            *reinterpret_cast<double2*>(winv + lane * WS + c) = make_double2(x[c], x[c + 1]);
-                    }
                     if (lane == 0 && f != 0 && sFail == 0) sFail = k0 + f;
+                } else if (warp == 1) {
+                    // W = L_kk^-1 (-> winv) by forward substitution, 8 pivots behind warp 0 (named barriers 1..3)
+                    warp_inverse<NBP, 8, WS>(lane, nrows, sRinv, winv, 1, [&](int k, int j) { return tile[TIDX(k, j)]; });
                 } else {
                     const int npan = (M + NBP - 1) / NBP, bps = (Nb + npan - 1) / npan;
                     const int ib0 = (k0 / NBP) * bps, ib1 = min(ib0 + bps, Nb);
-                    for (int i = ib0 + warp - 1; i < ib1; i += CS_WARPS - 1) {
+                    for (int i = ib0 + warp - 2; i < ib1; i += CS_WARPS - 2) {
                         const double xi = sR[3 * i], yi = sR[3 * i + 1], zi = sR[3 * i + 2];
                         double s0 = 0, s1 = 0, s2 = 0;
                         for (int j = lane; j < Nb; j += 32) {
@@ -503,7 +503,7 @@ size_t chain_step_smem(int M)
     const int NBP = 8 * NT, MP = (M + 7) & ~7;
     const size_t slot_d = ((size_t)(MP - NBP > NBP ? MP - NBP : NBP) * 4 + 15) & ~(size_t)15;
     return sizeof(double) * (CS_STAGES * slot_d + (size_t)(NBP / 4) * (MP + 1) * 4 + (size_t)NBP * (NBP + 4) + 4 * (size_t)MP +
-                             (MP + NBP) + 64 + 96);
+                             (MP + NBP) + 64 + 96 + 32);
 }
 
 }  // namespace

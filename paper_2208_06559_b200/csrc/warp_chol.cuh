@@ -1,26 +1,18 @@
-// warp_chol.cuh -- Cholesky factor AND inverse factor of one small SPD block (NB <= 32 rows) by ONE warp,
-// one matrix row per lane, everything in registers (Eq. 10, at block scale).
+// warp_chol.cuh -- the serial spine of the fused short-chain Cholesky: one small SPD block (NB <= 32 rows) is
+// factored by ONE warp, one matrix row per lane, in registers (Eq. 10, at block scale), while
+// a SECOND warp follows a few pivots behind and forms the inverse factor W = L^-1 by forward substitution.
 //
-// Why: the diagonal-block factorisation is the serial spine of every blocked Cholesky (M dependent pivots
-// per matrix).  The first version (a G x G thread grid, one CTA barrier and a full FP64 division per pivot)
-// took ~1100 cycles per pivot (profiles/r01_baseline_first_path.md).  Here the per-pivot dependency chain is
-//     SHFL (pivot broadcast) -> rsqrt (approx + one cubic correction) -> DMUL -> DFMA (next pivot, own lane)
-// ~ 100 cycles, and everything else (the rank-1 update of the trailing columns, the update of the inverse)
-// hangs off that chain: column k of L goes lane -> shared memory -> 16-byte broadcast loads.
-//
-// Right-looking elimination on x[] = row `lane`:   columns j > k hold the Schur complement a[lane][j],
-// columns c <= k hold the (unscaled) inverse of the unit-lower factor, w[lane][c] -- the two triangles never
-// overlap in time, so ONE register array of NB doubles carries both.  At pivot k
-//     l_ik = a_ik / sqrt(d_k)             (final column k of L, handed to store_l)
-//     a_ij -= l_ik l_jk                   (j > k)
-//     w_i. -= (l_ik / sqrt(d_k)) w_k.     (c < k),   w_ik = -l_ik / sqrt(d_k)
-// and at the end W = L^-1 has rows w_i. / sqrt(d_i).
+// Why: the diagonal-block factorisation is the serial part of every blocked Cholesky (M dependent pivots per
+// matrix).  Per pivot the dependency chain is
+//     SHFL (pivot broadcast) -> rsqrt (approx + one cubic correction + one Newton step) -> DMUL -> DFMA (next pivot)
+// ~ 130 cycles; everything else hangs off that chain.  Measured (profiles/r01_notes.md): a version that also
+// carried the inverse in the same warp executed ~95 instructions per pivot at IPC 0.2 (566 cycles per pivot) --
+// the time went into issue slots, not into the chain -- so the inverse moved to its own warp.
 #pragma once
 #include <cuda_runtime.h>
 
 // 1/sqrt(d), d > 0 normal: hardware seed (rsqrt.approx.ftz.f64, ~2^-20 or better) + one third-order step
-// y (1 + e/2 + 3 e^2/8), e = 1 - d y^2, and one Newton step on top -> <= 1 ulp-level error
-// (measured against rsqrt(): see tests).  9 dependent FP64 ops instead of the branchy library routine.
+// y (1 + e/2 + 3 e^2/8), e = 1 - d y^2, and one Newton step on top -> <= 1 ulp-level error.
 __device__ __forceinline__ double fast_rsqrt_pos(double d)
 {
     double y;
@@ -30,51 +22,44 @@ __device__ __forceinline__ double fast_rsqrt_pos(double d)
     double p = fma(0.375, e, 0.5);
     double q = e * p;
     y = fma(y, q, y);
-#ifndef BD_RSQRT_ONE_STEP
     t = d * y;
     e = fma(-t, y, 1.0);
     y = fma(0.5 * y, e, y);
-#endif
     return y;
 }
 
-// x[j]   in : A[lane][j] (symmetric block; only lanes < NB matter, lanes >= NB must hold zeros)
-//        out: W[lane][j] = (L^-1)[lane][j] for j <= lane, 0 for j > lane
-// s_col  : shared, 2*32 doubles, 16-byte aligned (column broadcast buffer, double buffered)
-// s_wrow : shared, NB rows of stride WS doubles (WS even, 16-byte aligned): scratch for the unscaled inverse rows
-// store_l(k, l): called by every lane at pivot k with l = L[lane][k] (valid for lane >= k)
-// returns 0, or 1 + the first pivot index with d <= 0 (or NaN); the results are then meaningless.
-template <int NB, int WS, class StoreL>
-__device__ __forceinline__ int warp_chol_inv(double (&x)[NB], const int lane, double* __restrict__ s_col,
-                                             double* __restrict__ s_wrow, StoreL&& store_l)
+// named-barrier producer / consumer pair (PTX ISA, bar.arrive / bar.sync example): the producer's shared-memory
+// stores before bar.arrive are visible to the consumer after its bar.sync on the same barrier
+__device__ __forceinline__ void named_arrive(int id, int nthreads) { asm volatile("bar.arrive %0, %1;\n" ::"r"(id), "r"(nthreads) : "memory"); }
+__device__ __forceinline__ void named_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(nthreads) : "memory"); }
+
+// Right-looking elimination on x[] = row `lane` of the symmetric block (lanes >= NB hold zeros):
+//     l_ik = a_ik / sqrt(d_k)   (column k of L, handed to store_l(k, l) by every lane, valid for lane >= k)
+//     a_ij -= l_ik l_jk         (j > k), l_jk broadcast through s_col (double buffered, one __syncwarp per pivot)
+// s_rinv[k] = 1/L_kk.  After pivots CH-1, 2CH-1, .. the warp arrives on named barrier bar0, bar0+1, .. (64 threads)
+// so that the inverse warp can start on the finished rows.  Returns 0 or 1 + the first pivot with d <= 0 (or NaN).
+template <int NB, int CH, class StoreL>
+__device__ __forceinline__ int warp_chol(double (&x)[NB], const int lane, double* __restrict__ s_col,
+                                         double* __restrict__ s_rinv, const int bar0, StoreL&& store_l)
 {
-    static_assert(NB <= 32 && (NB % 2) == 0 && (WS % 2) == 0, "warp_chol_inv: NB even, <= 32");
+    static_assert(NB <= 32 && (NB % 2) == 0 && (NB % CH) == 0, "warp_chol: NB even, <= 32, multiple of CH");
     int fail = 0;
-    double my_rinv = 1.0;
     double d = __shfl_sync(0xffffffffu, x[0], 0);
 #pragma unroll
     for (int k = 0; k < NB; ++k) {
-        // row k of the unscaled inverse (columns < k) is final: its owner publishes it
-        if (lane == k) {
-#pragma unroll
-            for (int c = 0; c < k; c += 2)
-                *reinterpret_cast<double2*>(s_wrow + k * WS + c) = make_double2(x[c], x[c + 1 < NB ? c + 1 : c]);
-        }
         if (!(d > 0.0) && fail == 0) fail = k + 1;
         const double rinv = fast_rsqrt_pos(d);
         const double l = x[k] * rinv;
-        if (lane == k) my_rinv = rinv;
-        store_l(k, l);
         if (k + 1 < NB) {                                   // next pivot first: it is the critical path
             const double dn = fma(-l, l, x[k + 1 < NB ? k + 1 : k]);
             d = __shfl_sync(0xffffffffu, dn, k + 1);
         }
+        store_l(k, l);
+        if (lane == k) s_rinv[k] = rinv;
         const double lm = (lane > k) ? l : 0.0;
         double* col = s_col + (k & 1) * 32;
         col[lane] = lm;
         __syncwarp();
-        const double m = lm * rinv;
-        // Schur complement columns j > k
         if ((k + 1) & 1) {
             if (k + 1 < NB) x[k + 1 < NB ? k + 1 : k] = fma(-lm, col[k + 1], x[k + 1 < NB ? k + 1 : k]);
 #pragma unroll
@@ -91,17 +76,35 @@ __device__ __forceinline__ int warp_chol_inv(double (&x)[NB], const int lane, do
                 x[j + 1] = fma(-lm, c2.y, x[j + 1]);
             }
         }
-        // inverse columns c < k, then the new column k
-#pragma unroll
-        for (int c = 0; c + 1 < k; c += 2) {
-            const double2 w2 = *reinterpret_cast<const double2*>(s_wrow + k * WS + c);
-            x[c] = fma(-m, w2.x, x[c]);
-            x[c + 1] = fma(-m, w2.y, x[c + 1]);
-        }
-        if (k & 1) x[k - 1 >= 0 ? k - 1 : 0] = fma(-m, s_wrow[k * WS + (k - 1 >= 0 ? k - 1 : 0)], x[k - 1 >= 0 ? k - 1 : 0]);
-        x[k] = (lane == k) ? 1.0 : -m;
+        if ((k + 1) % CH == 0) named_arrive(bar0 + k / CH, 64);
     }
-#pragma unroll
-    for (int c = 0; c < NB; ++c) x[c] *= my_rinv;
     return fail;
+}
+
+// Inverse factor by forward substitution, lane c = column c of W = L^-1 (lower):
+//     W[k][c] = (delta_kc - sum_{j<k} L[k][j] W[j][c]) / L[k][k]
+// L(k, j) (j < k) and s_rinv[k] come from shared memory as broadcast loads once the factoring warp has arrived on the
+// chunk's named barrier; rows k >= nrows (padding of a ragged block) are identity rows.  Row k goes to s_w[k*WS + c].
+template <int NB, int CH, int WS, class LoadL>
+__device__ __forceinline__ void warp_inverse(const int lane, const int nrows, const double* __restrict__ s_rinv,
+                                             double* __restrict__ s_w, const int bar0, LoadL&& L)
+{
+    double w[NB];
+#pragma unroll
+    for (int k = 0; k < NB; ++k) {
+        if (k % CH == 0) named_sync(bar0 + k / CH, 64);
+        double s0 = (lane == k) ? 1.0 : 0.0, s1 = 0.0;
+        if (k < nrows) {
+#pragma unroll
+            for (int j = 0; j + 1 < k; j += 2) {
+                s0 = fma(-L(k, j), w[j], s0);
+                s1 = fma(-L(k, j + 1), w[j + 1], s1);
+            }
+            if (k & 1) s0 = fma(-L(k, k - 1 >= 0 ? k - 1 : 0), w[k - 1 >= 0 ? k - 1 : 0], s0);
+            w[k] = (s0 + s1) * s_rinv[k];
+        } else {
+            w[k] = s0;
+        }
+        if (lane < NB) s_w[k * WS + lane] = w[k];
+    }
 }
