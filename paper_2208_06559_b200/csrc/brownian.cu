@@ -65,6 +65,84 @@ __global__ void __launch_bounds__(kTrmvWarps * 32) k_trmv(int M, const double* _
     if (lane == 0) y_all[(size_t)c * M + row] = s;
 }
 
+// Variant for LONG chains (M > TRMV_STAGED_MIN_M).  A CTA takes a block of 32 adjacent rows, four rows per warp; the
+// blocks with the longest rows are scheduled first.  dW is staged through shared
+// memory in chunks of TRMV_CHUNK columns, double buffered, and re-used by all rows of the CTA: at M = 30003 the
+// vector (240 KB) no longer fits in L1 and the first version (one row per warp, dW from global memory) fetched as
+// many bytes of dW from L2 as of L from HBM (4.27 TB/s at c5 against 5.1 TB/s at c4; this variant: 4.58 TB/s at c5, but
+// 4.5 TB/s at c3/c4 where the one-row-per-warp kernel is faster -- the barrier per chunk costs more than L1 misses there).  Lanes read 16-byte pairs of
+// four rows: 8 independent 16-byte loads in flight per lane.
+constexpr int TRMV_STAGED_MIN_M = 16384;   // dW of 128 KB still lives in L1 beside the row streams
+constexpr int TRMV_WARPS = 8, TRMV_RPW = 4, TRMV_BLK = TRMV_WARPS * TRMV_RPW, TRMV_CHUNK = 2048;
+
+__global__ void __launch_bounds__(TRMV_WARPS * 32) k_trmv_staged(int M, const double* __restrict__ L_all, int64_t ld, int64_t stride,
+                                                         const double* __restrict__ dW_all, double* __restrict__ y_all)
+{
+    __shared__ __align__(16) double s_w[2][TRMV_CHUNK];
+    const int c = blockIdx.y;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nblk = (M + TRMV_BLK - 1) / TRMV_BLK;
+    const int blk = nblk - 1 - blockIdx.x;                                      // longest rows are scheduled first
+    const bool idle = false;
+    const int row0 = blk * TRMV_BLK + warp * TRMV_RPW;
+    const double* Lc = L_all + (size_t)c * stride;
+    const double* dW = dW_all + (size_t)c * M;
+    const int ncols_cta = min(M, (blk + 1) * TRMV_BLK);                         // longest row of the CTA + 1
+
+    int n[TRMV_RPW];
+    const double* Lr[TRMV_RPW];
+    double acc[TRMV_RPW];
+#pragma unroll
+    for (int r = 0; r < TRMV_RPW; ++r) {
+        const int row = row0 + r;
+        n[r] = (idle || row >= M) ? 0 : row + 1;
+        Lr[r] = Lc + (size_t)min(row, M - 1) * ld;
+        acc[r] = 0.0;
+    }
+    const int nmax = n[TRMV_RPW - 1] > 0 ? n[TRMV_RPW - 1] : max(max(n[0], n[1]), n[2]);   // rows grow with r
+
+    auto stage = [&](int ch, int buf) {
+        const int j0 = ch * TRMV_CHUNK;
+        for (int j = threadIdx.x; j < TRMV_CHUNK; j += TRMV_WARPS * 32) s_w[buf][j] = (j0 + j < M) ? dW[j0 + j] : 0.0;
+    };
+    const int nch = (ncols_cta + TRMV_CHUNK - 1) / TRMV_CHUNK;
+    stage(0, 0);
+    __syncthreads();
+    for (int ch = 0; ch < nch; ++ch) {
+        if (ch + 1 < nch) stage(ch + 1, (ch + 1) & 1);
+        const int j0 = ch * TRMV_CHUNK;
+        const int jend = min(nmax - j0, TRMV_CHUNK);                            // columns of this chunk this warp needs
+        const double* w = s_w[ch & 1];
+        for (int j = 2 * lane; j < jend; j += 128) {
+            double2 l[2][TRMV_RPW];
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+#pragma unroll
+                for (int r = 0; r < TRMV_RPW; ++r) {
+                    const int col = j0 + j + 64 * u;
+                    l[u][r] = (col < n[r]) ? *reinterpret_cast<const double2*>(Lr[r] + col) : make_double2(0.0, 0.0);
+                }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int jj = j + 64 * u;
+                const double2 wv = (jj < TRMV_CHUNK) ? *reinterpret_cast<const double2*>(w + jj) : make_double2(0.0, 0.0);
+#pragma unroll
+                for (int r = 0; r < TRMV_RPW; ++r) {
+                    const int col = j0 + jj;
+                    const double ly = (col + 1 < n[r]) ? l[u][r].y : 0.0;        // the pair may straddle the diagonal
+                    acc[r] += l[u][r].x * wv.x + ly * wv.y;
+                }
+            }
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int r = 0; r < TRMV_RPW; ++r) {
+        const double s = warp_sum(acc[r]);
+        if (lane == 0 && n[r] > 0) y_all[(size_t)c * M + row0 + r] = s;
+    }
+}
+
 }  // namespace
 
 int bdk_noise(bd_ctx* ctx, uint64_t step, double* dW)
@@ -77,6 +155,11 @@ int bdk_noise(bd_ctx* ctx, uint64_t step, double* dW)
 
 int bdk_trmv(bd_ctx* ctx, const double* L, int64_t ld, int64_t stride, const double* dW, double* y)
 {
+    if (ctx->M > TRMV_STAGED_MIN_M) {
+        const int nb = (ctx->M + TRMV_BLK - 1) / TRMV_BLK;
+        BD_LAUNCH(ctx, k_trmv_staged, dim3(nb, ctx->C), dim3(TRMV_WARPS * 32), 0, ctx->M, L, ld, stride, dW, y);
+        return 0;
+    }
     const int nblk = (ctx->M + kTrmvWarps - 1) / kTrmvWarps;
     BD_LAUNCH(ctx, k_trmv, dim3(nblk, ctx->C), dim3(kTrmvWarps * 32), 0, ctx->M, L, ld, stride, dW, y);
     return 0;
