@@ -441,7 +441,8 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
         attr_set = true;
     }
     const int n = ctx->M, C = ctx->C;
-    const int NB = (n >= 8192) ? 512 : 256;
+    // outer panel width, from a sweep on B200 (profiles/r01_summary.md): flat within ~2 % between 256 and 1024
+    const int NB = (n >= 8192) ? 1024 : (n >= 4096) ? 512 : 256;
     for (int J = 0; J < n; J += NB) {
         const int Jend = (J + NB < n) ? J + NB : n;
         for (int j = J; j < Jend; j += BD_NB_INNER) {
