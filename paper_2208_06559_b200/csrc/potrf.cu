@@ -249,7 +249,12 @@ __global__ void __launch_bounds__(256, 2) k_trsm(double* __restrict__ A_all, int
 //     load cursor is STAGES-1 k-slabs ahead of the compute cursor and simply moves on to the next tile.
 //   smem rows are padded to 20 doubles so the 8-byte fragment loads of a warp fall in distinct banks.
 // =================================================================================================
-constexpr int BM = 128, BN = 128, BK = 16, STAGES = 4, SLD = 20;
+#ifndef SYRK_BK
+#define SYRK_BK 32
+#define SYRK_STAGES 2
+#endif
+constexpr int BM = 128, BN = 128, BK = SYRK_BK, STAGES = SYRK_STAGES, SLD = BK + 4;
+constexpr int CPR = BK / 2, RPP = 256 / CPR;          // 16-byte chunks per slab row, rows copied per pass of the CTA
 constexpr int SYRK_SMEM = STAGES * (BM + BN) * SLD * (int)sizeof(double);
 
 struct SyrkArgs {
@@ -291,30 +296,40 @@ __global__ void __launch_bounds__(256, 1) k_syrk(const SyrkArgs a)
     const int64_t ld = a.ld;
 
     // ---- load cursor (runs STAGES-1 slabs ahead of the compute cursor) -----------------------------
+    // Per tile, each thread keeps ONE source pointer per operand (its first row, clamped into the matrix) and the
+    // row stride between its passes; per slab a copy then costs one 64-bit add (the first version recomputed
+    // chain * stride + row * ld per copy: ~120 integer instructions per slab in front of the DMMAs).
     int l_idx = blockIdx.x, l_kt = 0, l_tm0 = 0, l_tn0 = 0, l_chain = 0;
-    if (l_idx < a.total) syrk_tile(a, l_idx, l_chain, l_tm0, l_tn0);
-    const int lrow = tid >> 3, lch = tid & 7;            // this thread copies rows lrow, lrow+32, .. chunk lch
+    const int lrow = tid / CPR, lch = tid % CPR;         // this thread copies rows lrow, lrow+RPP, .. chunk lch
+    const int64_t pass_stride = (int64_t)RPP * ld;       // doubles between the rows of two passes
+    const double* pA = a.A;
+    const double* pB = a.A;
+    auto set_tile = [&]() {
+        syrk_tile(a, l_idx, l_chain, l_tm0, l_tn0);
+        const double* base = a.A + (size_t)l_chain * a.stride + a.k_lo + 2 * lch;
+        pA = base + (size_t)min(l_tm0 + lrow, a.m_hi - 1) * ld;
+        pB = base + (size_t)min(l_tn0 + lrow, a.n_hi - 1) * ld;
+    };
+    if (l_idx < a.total) set_tile();
     auto load_next = [&](int slot) {
         if (l_idx < a.total) {
-            const double* src_k = a.A + (size_t)l_chain * a.stride + a.k_lo + l_kt * BK + 2 * lch;
+            const int kofs = l_kt * BK;
             double* dA = sA + ((size_t)slot * BM + lrow) * SLD + 2 * lch;
             double* dB = sB + ((size_t)slot * BN + lrow) * SLD + 2 * lch;
 #pragma unroll
-            for (int it = 0; it < BM / 32; ++it) {
-                const int gr = l_tm0 + lrow + 32 * it;
-                const bool ok = gr < a.m_hi;
-                cp_async16(dA + (size_t)it * 32 * SLD, src_k + (size_t)(ok ? gr : a.m_hi - 1) * ld, ok ? 16 : 0);
+            for (int it = 0; it < BM / RPP; ++it) {
+                const bool ok = l_tm0 + lrow + RPP * it < a.m_hi;
+                cp_async16(dA + (size_t)it * RPP * SLD, pA + kofs + (ok ? it * pass_stride : 0), ok ? 16 : 0);
             }
 #pragma unroll
-            for (int it = 0; it < BN / 32; ++it) {
-                const int gr = l_tn0 + lrow + 32 * it;
-                const bool ok = gr < a.n_hi;
-                cp_async16(dB + (size_t)it * 32 * SLD, src_k + (size_t)(ok ? gr : a.n_hi - 1) * ld, ok ? 16 : 0);
+            for (int it = 0; it < BN / RPP; ++it) {
+                const bool ok = l_tn0 + lrow + RPP * it < a.n_hi;
+                cp_async16(dB + (size_t)it * RPP * SLD, pB + kofs + (ok ? it * pass_stride : 0), ok ? 16 : 0);
             }
             if (++l_kt == KT) {
                 l_kt = 0;
                 l_idx += gridDim.x;
-                if (l_idx < a.total) syrk_tile(a, l_idx, l_chain, l_tm0, l_tn0);
+                if (l_idx < a.total) set_tile();
             }
         }
     };
@@ -443,8 +458,17 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
     const int n = ctx->M, C = ctx->C;
     // outer panel width, from a sweep on B200 (profiles/r01_summary.md): flat within ~2 % between 256 and 1024
     const int NB = (n >= 8192) ? 1024 : (n >= 4096) ? 512 : 256;
+    // Outer level: LEFT-looking for short matrices (block column J is brought up to date by all finished columns in
+    // one pass, K = J: each C tile goes through the accumulators once per factorisation), RIGHT-looking otherwise
+    // (measured on B200: c3 0.483 -> 0.493 of peak with left-looking, c4 equal, c5 0.738 -> 0.696: the K-deep operand
+    // streams of all row blocks then no longer share L2).
+    const bool left = n < 4096;
     for (int J = 0; J < n; J += NB) {
         const int Jend = (J + NB < n) ? J + NB : n;
+        if (left && J > 0) {
+            int rc = launch_syrk(ctx, A, ld, stride, J, n, Jend, 0, J);
+            if (rc != 0) return rc;
+        }
         for (int j = J; j < Jend; j += BD_NB_INNER) {
             const int nloc = (n - j < BD_NB_INNER) ? n - j : BD_NB_INNER;
             BD_LAUNCH(ctx, k_potf2, dim3(C), dim3(256), 0, A, ld, stride, j, nloc, info, ctx->Winv);
@@ -458,7 +482,7 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
                 }
             }
         }
-        if (Jend < n) {
+        if (!left && Jend < n) {
             int rc = launch_syrk(ctx, A, ld, stride, Jend, n, n, J, Jend - J);
             if (rc != 0) return rc;
         }
