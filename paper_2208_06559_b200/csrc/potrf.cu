@@ -2,12 +2,12 @@
 // batched over chains.  The paper calls cusolverDnDpotrf once per chain per step (:172); this is a
 // hand-written blocked right-looking factorisation for sm_100a:
 //
-//   two-level blocking: outer panels of NB columns, inner diagonal blocks of 64 columns
-//     k_potf2   64x64 diagonal block, register-resident, one CTA per chain
-//     k_trsm    rows below the diagonal block:  X L_jj^T = A   (one thread per row, L_jj broadcast from smem)
-//     k_syrk    C -= P P^T with FP64 tensor-core DMMA (mma.sync m8n8k4), 128x128 tiles, 4-stage cp.async
-//               pipeline; used both for the in-panel update (K = 64) and the trailing update (K = NB),
-//               so the trailing matrix is read and written once per NB columns, not once per 64.
+//   outer panels of NB columns (right-looking trailing update, K = NB), each factored RECURSIVELY (left half,
+//   update of the right half with K = half, right half) down to 64-column diagonal blocks:
+//     k_potf2   64x64 diagonal block, register-resident, one CTA per chain, also forms W = L_jj^-1
+//     k_trsm    rows below the diagonal block:  X = A W^T on the tensor cores
+//     k_syrk    C -= P P^T with FP64 tensor-core DMMA (mma.sync m8n8k4), 128x128 tiles, cp.async operand
+//               pipeline; K = 64, 128, 256, .. inside a panel, K = NB for the trailing update.
 //
 // FP64 has no tcgen05 kind; the FP64 tensor path on sm_100a is warp-level DMMA (measured 37.07
 // TFLOP/s on B200), so operands go global -> cp.async -> padded smem -> registers.
@@ -245,15 +245,18 @@ __global__ void __launch_bounds__(256, 2) k_trsm(double* __restrict__ A_all, int
 //     when it ends: acc = -C + P P^T.  No load of C depends on anything in the epilogue, so the tensor
 //     pipe never waits on a DRAM round trip there (the first version's epilogue took 28 % of the
 //     kernel, profiles/r01_baseline_first_path.md); the next tile's C is prefetched into L2 meanwhile.
-//   - the operand pipeline (4-stage cp.async ring of 128 x 16 slabs) runs ACROSS tile boundaries: the
+//   - the operand pipeline (cp.async ring of 128 x BK slabs, BK = 32, 2 stages) runs ACROSS tile boundaries: the
 //     load cursor is STAGES-1 k-slabs ahead of the compute cursor and simply moves on to the next tile.
-//   smem rows are padded to 20 doubles so the 8-byte fragment loads of a warp fall in distinct banks.
+//   smem rows are padded to BK + 8 doubles: the 16-byte fragment loads (two k-steps each) are conflict free.
 // =================================================================================================
 #ifndef SYRK_BK
 #define SYRK_BK 32
 #define SYRK_STAGES 2
 #endif
-constexpr int BM = 128, BN = 128, BK = SYRK_BK, STAGES = SYRK_STAGES, SLD = BK + 4;
+#ifndef SYRK_BN
+#define SYRK_BN 128
+#endif
+constexpr int BM = 128, BN = SYRK_BN, NTW = BN / 16, SYRK_CTAS = (BN == 64) ? 2 : 1, BK = SYRK_BK, STAGES = SYRK_STAGES, SLD = BK + 8;   // SLD % 16 == 8: conflict-free 16-byte fragment loads
 constexpr int CPR = BK / 2, RPP = 256 / CPR;          // 16-byte chunks per slab row, rows copied per pass of the CTA
 constexpr int SYRK_SMEM = STAGES * (BM + BN) * SLD * (int)sizeof(double);
 
@@ -261,7 +264,7 @@ struct SyrkArgs {
     double* A;
     int64_t ld, stride;
     int lo, m_hi, n_hi, k_lo, K;     // rows [lo, m_hi), columns [lo, n_hi), inner range [k_lo, k_lo+K)
-    int TN, tri, per_chain, total;   // tile columns, TN(TN+1)/2, tiles per chain, tiles in the launch
+    int TN, T2, tri, per_chain, total;   // tile columns, triangular tile rows, tiles in them, tiles per chain / launch
 };
 
 // tile index -> (chain, first row, first column).  Tiles (ty, tx), tx <= ty, tx < TN, row-major within a chain.
@@ -269,22 +272,25 @@ __device__ __forceinline__ void syrk_tile(const SyrkArgs& a, int idx, int& chain
 {
     chain = idx / a.per_chain;
     const int t = idx - chain * a.per_chain;
+    // row ty of tiles has min(TN, R (ty + 1)) column tiles, R = BM / BN (tiles up to and including the diagonal)
+    constexpr int R = BM / BN;
     int ty, tx;
     if (t < a.tri) {
-        ty = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
-        while ((ty + 1) * (ty + 2) / 2 <= t) ++ty;
-        while (ty * (ty + 1) / 2 > t) --ty;
-        tx = t - ty * (ty + 1) / 2;
+        // rows 0 .. T2-1 are triangular: R (ty+1) tiles each, R ty (ty+1) / 2 before row ty
+        ty = (int)((sqrt(8.0 * (double)t / R + 1.0) - 1.0) * 0.5);
+        while (R * (ty + 1) * (ty + 2) / 2 <= t) ++ty;
+        while (R * ty * (ty + 1) / 2 > t) --ty;
+        tx = t - R * ty * (ty + 1) / 2;
     } else {
         const int u = t - a.tri;
-        ty = a.TN + u / a.TN;
+        ty = a.T2 + u / a.TN;
         tx = u - (u / a.TN) * a.TN;
     }
     tm0 = a.lo + ty * BM;
     tn0 = a.lo + tx * BN;
 }
 
-__global__ void __launch_bounds__(256, 1) k_syrk(const SyrkArgs a)
+__global__ void __launch_bounds__(256, SYRK_CTAS) k_syrk(const SyrkArgs a)
 {
     extern __shared__ __align__(16) double smem[];
     double* sA = smem;                                   // [STAGES][BM][SLD]
@@ -346,7 +352,7 @@ __global__ void __launch_bounds__(256, 1) k_syrk(const SyrkArgs a)
         syrk_tile(a, idx, chain, tm0, tn0);
         double* A = a.A + (size_t)chain * a.stride;
         // this warp's 32 x 64 block lies entirely above the diagonal -> no arithmetic (still loads/syncs)
-        const bool warp_active = (tn0 + wn * 64) <= (tm0 + wm * 32 + 31);
+        const bool warp_active = (tn0 + wn * (BN / 2)) <= (tm0 + wm * 32 + 31);
 
         // L2 prefetch of the NEXT tile's C (128 rows x 1 KB): its loads then cost an L2 hit, not a DRAM trip
         if (idx + (int)gridDim.x < a.total) {
@@ -354,22 +360,22 @@ __global__ void __launch_bounds__(256, 1) k_syrk(const SyrkArgs a)
             syrk_tile(a, idx + gridDim.x, nc, nm0, nn0);
             const double* Cn = a.A + (size_t)nc * a.stride;
 #pragma unroll
-            for (int it = 0; it < 4; ++it) {
+            for (int it = 0; it < BN / 32; ++it) {
                 const int q = tid + 256 * it;
-                const int gr = nm0 + (q >> 3), gc = nn0 + (q & 7) * 16;
+                const int gr = nm0 + q / (BN / 16), gc = nn0 + (q % (BN / 16)) * 16;
                 if (gr < a.m_hi && gc <= gr && gc < a.n_hi) prefetch_l2(Cn + (size_t)gr * ld + gc);
             }
         }
 
-        double acc[4][8][2];
+        double acc[4][NTW][2];
         if (warp_active) {
 #pragma unroll
             for (int mt = 0; mt < 4; ++mt) {
                 const int gi = tm0 + wm * 32 + mt * 8 + g;
                 const double* crow = A + (size_t)gi * ld;
 #pragma unroll
-                for (int nt = 0; nt < 8; ++nt) {
-                    const int gj = tn0 + wn * 64 + nt * 8 + 2 * t;
+                for (int nt = 0; nt < NTW; ++nt) {
+                    const int gj = tn0 + wn * (BN / 2) + nt * 8 + 2 * t;
                     double c0 = 0.0, c1 = 0.0;
                     if (gi < a.m_hi) {
                         if (gj + 1 < a.n_hi && gj + 1 <= gi) {
@@ -391,19 +397,26 @@ __global__ void __launch_bounds__(256, 1) k_syrk(const SyrkArgs a)
             load_next((git + STAGES - 1) % STAGES);
             cp_async_commit();
             if (warp_active) {
-                const double* a_base = sA + ((size_t)(git % STAGES) * BM + wm * 32 + g) * SLD + t;
-                const double* b_base = sB + ((size_t)(git % STAGES) * BN + wn * 64 + g) * SLD + t;
+                // One 16-byte load per fragment row and PAIR of k-steps: within a group of 8 columns k-step 0 takes the
+                // even columns (.x of lane t = column 2t), k-step 1 the odd ones (.y).  A and B use the same column
+                // permutation, so the sum over k is the same set of products; half the shared-memory load instructions.
+                const double* a_base = sA + ((size_t)(git % STAGES) * BM + wm * 32 + g) * SLD + 2 * t;
+                const double* b_base = sB + ((size_t)(git % STAGES) * BN + wn * (BN / 2) + g) * SLD + 2 * t;
 #pragma unroll
-                for (int ks = 0; ks < BK / 4; ++ks) {
-                    double af[4], bf[8];
+                for (int k8 = 0; k8 < BK / 8; ++k8) {
+                    double2 af[4], bf[NTW];
 #pragma unroll
-                    for (int mt = 0; mt < 4; ++mt) af[mt] = a_base[mt * 8 * SLD + ks * 4];
+                    for (int mt = 0; mt < 4; ++mt) af[mt] = *reinterpret_cast<const double2*>(a_base + mt * 8 * SLD + k8 * 8);
 #pragma unroll
-                    for (int nt = 0; nt < 8; ++nt) bf[nt] = b_base[nt * 8 * SLD + ks * 4];
+                    for (int nt = 0; nt < NTW; ++nt) bf[nt] = *reinterpret_cast<const double2*>(b_base + nt * 8 * SLD + k8 * 8);
 #pragma unroll
                     for (int mt = 0; mt < 4; ++mt)
 #pragma unroll
-                        for (int nt = 0; nt < 8; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], af[mt], bf[nt]);
+                        for (int nt = 0; nt < NTW; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], af[mt].x, bf[nt].x);
+#pragma unroll
+                    for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                        for (int nt = 0; nt < NTW; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], af[mt].y, bf[nt].y);
                 }
             }
         }
@@ -414,8 +427,8 @@ __global__ void __launch_bounds__(256, 1) k_syrk(const SyrkArgs a)
                 if (gi >= a.m_hi) continue;
                 double* crow = A + (size_t)gi * ld;
 #pragma unroll
-                for (int nt = 0; nt < 8; ++nt) {
-                    const int gj = tn0 + wn * 64 + nt * 8 + 2 * t;
+                for (int nt = 0; nt < NTW; ++nt) {
+                    const int gj = tn0 + wn * (BN / 2) + nt * 8 + 2 * t;
                     if (gj + 1 < a.n_hi && gj + 1 <= gi) {
                         *reinterpret_cast<double2*>(crow + gj) = make_double2(-acc[mt][nt][0], -acc[mt][nt][1]);
                     } else if (gj < a.n_hi && gj <= gi) {
@@ -436,10 +449,13 @@ int launch_syrk(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int lo, int 
     a.lo = lo; a.m_hi = m_hi; a.n_hi = n_hi; a.k_lo = k_lo; a.K = K;
     const int TM = (m_hi - lo + BM - 1) / BM;
     a.TN = (n_hi - lo + BN - 1) / BN;
-    a.tri = a.TN * (a.TN + 1) / 2;
-    a.per_chain = a.tri + (TM - a.TN) * a.TN;
+    constexpr int R = BM / BN;
+    a.T2 = a.TN / R;                                     // tile rows that end at the diagonal: R (ty + 1) tiles each
+    a.tri = R * a.T2 * (a.T2 + 1) / 2;
+    a.per_chain = a.tri + (TM - a.T2) * a.TN;
     a.total = a.per_chain * ctx->C;
-    const int grid = a.total < ctx->num_sms ? a.total : ctx->num_sms;
+    const int slots = SYRK_CTAS * ctx->num_sms;
+    const int grid = a.total < slots ? a.total : slots;
     BD_LAUNCH(ctx, k_syrk, dim3(grid), dim3(256), SYRK_SMEM, a);
     return 0;
 }
@@ -456,34 +472,47 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
         attr_set = true;
     }
     const int n = ctx->M, C = ctx->C;
-    // outer panel width, from a sweep on B200 (profiles/r01_summary.md): flat within ~2 % between 256 and 1024
-    const int NB = (n >= 8192) ? 1024 : (n >= 4096) ? 512 : 256;
-    // Outer level: LEFT-looking for short matrices (block column J is brought up to date by all finished columns in
-    // one pass, K = J: each C tile goes through the accumulators once per factorisation), RIGHT-looking otherwise
-    // (measured on B200: c3 0.483 -> 0.493 of peak with left-looking, c4 equal, c5 0.738 -> 0.696: the K-deep operand
-    // streams of all row blocks then no longer share L2).
-    const bool left = n < 4096;
+    // outer panel width, from sweeps on B200 (profiles/r01_summary.md): with the recursive panel below, wide outer
+    // panels win (c4: 256 -> 0.641, 1024 -> 0.688, 4096 -> 0.695 of peak; c5: 0.686 / 0.769 / 0.781)
+    const int NB = (n >= 4096) ? 4096 : 1024;
+    // Outer level: right-looking.  A left-looking outer loop (block column J updated by all finished columns in one
+    // pass, K = J; kept behind `left`) measured equal at c3 / c4 and slower at c5 (0.78 -> 0.75: the K-deep operand
+    // streams of all row blocks no longer share L2).
+    const bool left = false;
+    // In-panel factorisation of columns [J0, J1), all rows below included, RECURSIVELY: left half, update of the
+    // right half with K = (J1 - J0) / 2, right half.  Against a plain right-looking sweep of 64-column blocks (every
+    // block updated once per preceding block, always K = 64, DMMA pipe ~50 % busy) each column block now sees
+    // log2((J1 - J0) / 64) updates with K = 64, 128, 256, ..
+    struct Rec {
+        bd_ctx* ctx; double* A; int64_t ld, stride; int32_t* info; int n, C, trsm_smem;
+        int run(int J0, int J1)
+        {
+            if (J1 - J0 <= BD_NB_INNER) {
+                const int nloc = J1 - J0;
+                BD_LAUNCH(ctx, k_potf2, dim3(C), dim3(256), 0, A, ld, stride, J0, nloc, info, ctx->Winv);
+                if (J1 < n)
+                    BD_LAUNCH(ctx, k_trsm, dim3((n - J1 + TRSM_ROWS - 1) / TRSM_ROWS, C), dim3(256), trsm_smem, A, ld, stride, J0,
+                              J1, n, ctx->Winv);
+                return 0;
+            }
+            const int half = ((J1 - J0) / 2 + BD_NB_INNER - 1) / BD_NB_INNER * BD_NB_INNER;
+            const int mid = J0 + half;
+            int rc = run(J0, mid);
+            if (rc != 0) return rc;
+            if ((rc = launch_syrk(ctx, A, ld, stride, mid, n, J1, J0, half)) != 0) return rc;
+            return run(mid, J1);
+        }
+    } rec{ctx, A, ld, stride, info, n, C, trsm_smem};
     for (int J = 0; J < n; J += NB) {
         const int Jend = (J + NB < n) ? J + NB : n;
         if (left && J > 0) {
             int rc = launch_syrk(ctx, A, ld, stride, J, n, Jend, 0, J);
             if (rc != 0) return rc;
         }
-        for (int j = J; j < Jend; j += BD_NB_INNER) {
-            const int nloc = (n - j < BD_NB_INNER) ? n - j : BD_NB_INNER;
-            BD_LAUNCH(ctx, k_potf2, dim3(C), dim3(256), 0, A, ld, stride, j, nloc, info, ctx->Winv);
-            const int r_lo = j + BD_NB_INNER;
-            if (r_lo < n) {
-                BD_LAUNCH(ctx, k_trsm, dim3((n - r_lo + TRSM_ROWS - 1) / TRSM_ROWS, C), dim3(256), trsm_smem, A, ld, stride, j,
-                          r_lo, n, ctx->Winv);
-                if (r_lo < Jend) {
-                    int rc = launch_syrk(ctx, A, ld, stride, r_lo, n, Jend, j, BD_NB_INNER);
-                    if (rc != 0) return rc;
-                }
-            }
-        }
+        int rc = rec.run(J, Jend);
+        if (rc != 0) return rc;
         if (!left && Jend < n) {
-            int rc = launch_syrk(ctx, A, ld, stride, Jend, n, n, J, Jend - J);
+            rc = launch_syrk(ctx, A, ld, stride, Jend, n, n, J, Jend - J);
             if (rc != 0) return rc;
         }
     }
