@@ -1,0 +1,114 @@
+// potf2_blocked.cuh -- k_potf2: Cholesky factor AND inverse factor of one nb x nb (nb <= 64) diagonal block per
+// chain (Eq. 10, at block scale), the serial step between two tensor-core phases of bdk_potrf.
+//
+// The block is split 32 + 32:   A = [A11 . ; A21 A22]
+//   1. L11 = chol(A11) by warp 0 (one row per lane, registers + shuffles, warp_chol.cuh) while warp 1 forms
+//      W11 = L11^-1 by forward substitution 8 pivots behind it
+//   2. L21 = A21 W11^T                      (all 256 threads, 4 outputs each, operands in shared memory)
+//   3. A22 -= L21 L21^T
+//   4. L22 = chol(A22), W22 = L22^-1        (as step 1)
+//   5. W21 = -W22 (L21 W11)
+// The first version eliminated all 64 pivots with one CTA barrier per pivot and then inverted with 64 threads
+// (37 us at c4, 66 us at c3 where 172 registers allowed one CTA per SM only); here the 64 dependent pivots run
+// at the warp-level chain latency.  A non-positive (or NaN) pivot records info = 1-based global row.
+#pragma once
+#include "bd_internal.cuh"
+#include "warp_chol.cuh"
+
+namespace potf2 {
+
+constexpr int HB = 32;            // half block
+constexpr int SLDP = 65;          // row stride of the 64 x 64 working copies (odd: conflict-free columns)
+
+// out[c] = sum_p X[i][p] * Y(j, p), j = jq + c, c = 0..3: product of two 32 x 32 operands held in shared memory;
+// yt selects Y(j, p) = Y[p][j] (plain product X Y) or Y[j][p] (X Y^T).  Triangular operands carry explicit zeros.
+__device__ __forceinline__ void gemm32(const double* __restrict__ X, const double* __restrict__ Y, bool yt, int i, int jq,
+                                       double (&out)[4])
+{
+#pragma unroll
+    for (int c = 0; c < 4; ++c) out[c] = 0.0;
+#pragma unroll 8
+    for (int p = 0; p < HB; ++p) {
+        const double x = X[i * SLDP + p];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) out[c] = fma(x, yt ? Y[p * SLDP + jq + c] : Y[(jq + c) * SLDP + p], out[c]);
+    }
+}
+
+constexpr int SMEM_BYTES = (2 * 64 * SLDP + 128) * (int)sizeof(double);
+
+__global__ void __launch_bounds__(256) k_potf2(double* __restrict__ A_all, int64_t ld, int64_t stride, int j0, int nloc,
+                                               int32_t* __restrict__ info, double* __restrict__ Winv)
+{
+    extern __shared__ __align__(16) double sm[];
+    double* S = sm;                       // [64][SLDP] the block, then L (lower, zeros above the diagonal)
+    double* Wm = S + 64 * SLDP;           // [64][SLDP] W = L^-1
+    double* sCol = Wm + 64 * SLDP;        // [64] column broadcast buffer of warp_chol
+    double* sRinv = sCol + 64;            // [64] 1 / L_kk
+    __shared__ int sFail;
+    const int c = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    double* A = A_all + (size_t)c * stride + (size_t)j0 * ld + j0;
+    for (int idx = tid; idx < 64 * 64; idx += 256) {
+        const int i = idx >> 6, j = idx & 63;
+        double v = (i == j) ? 1.0 : 0.0;                           // identity padding for a ragged block
+        if (i < nloc && j <= i) v = A[(size_t)i * ld + j];
+        S[i * SLDP + j] = (j <= i) ? v : 0.0;
+        Wm[i * SLDP + j] = 0.0;
+    }
+    if (tid == 0) sFail = 0;
+    __syncthreads();
+
+    auto factor_half = [&](int o) {                                // rows / columns o .. o+31
+        if (warp == 0) {
+            double x[HB];
+#pragma unroll
+            for (int j = 0; j < HB; ++j) x[j] = S[(o + max(lane, j)) * SLDP + o + min(lane, j)];
+            __syncwarp();
+            const int f = warp_chol<HB, 8>(x, lane, sCol, sRinv + o, 1, [&](int k, double l) {
+                S[(o + lane) * SLDP + o + k] = (lane >= k) ? l : 0.0;
+            });
+            if (lane == 0 && f != 0 && sFail == 0) sFail = j0 + o + f;
+        } else if (warp == 1) {
+            warp_inverse<HB, 8, SLDP>(lane, HB, sRinv + o, Wm + o * SLDP + o, 1, [&](int k, int j) { return S[(o + k) * SLDP + o + j]; });
+        }
+    };
+    const int i = tid >> 3, jq = (tid & 7) * 4;
+    double out[4];
+
+    factor_half(0);
+    __syncthreads();
+    if (nloc > HB) {
+        gemm32(S + HB * SLDP, Wm, false, i, jq, out);              // L21 = A21 W11^T
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 4; ++q) S[(HB + i) * SLDP + jq + q] = out[q];
+        __syncthreads();
+        gemm32(S + HB * SLDP, S + HB * SLDP, false, i, jq, out);   // A22 -= L21 L21^T (lower part)
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            if (jq + q <= i) S[(HB + i) * SLDP + HB + jq + q] -= out[q];
+        __syncthreads();
+        factor_half(HB);
+        __syncthreads();
+        gemm32(S + HB * SLDP, Wm, true, i, jq, out);               // T = L21 W11 -> the (still empty) W21 area
+#pragma unroll
+        for (int q = 0; q < 4; ++q) Wm[(HB + i) * SLDP + jq + q] = out[q];
+        __syncthreads();
+        gemm32(Wm + HB * SLDP + HB, Wm + HB * SLDP, true, i, jq, out);   // W21 = -W22 T
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 4; ++q) Wm[(HB + i) * SLDP + jq + q] = -out[q];
+        __syncthreads();
+    }
+    if (tid == 0 && sFail != 0 && info != nullptr && info[c] == 0) info[c] = sFail;
+    for (int idx = tid; idx < 64 * 64; idx += 256) {
+        const int r = idx >> 6, j = idx & 63;
+        if (r < nloc && j <= r) A[(size_t)r * ld + j] = S[r * SLDP + j];
+    }
+    if (Winv != nullptr && nloc == 64) {
+        double* W = Winv + (size_t)c * 64 * 64;
+        for (int idx = tid; idx < 64 * 64; idx += 256) W[idx] = Wm[(idx >> 6) * SLDP + (idx & 63)];
+    }
+}
+
+}  // namespace potf2

@@ -14,6 +14,7 @@
 // Matrices are ROW-major, lower triangle: L[i][j], j <= i, so both SYRK operands are K-contiguous
 // rows of the same panel ("NT" form) and the DMMA A and B fragments use the same access pattern.
 #include "bd_internal.cuh"
+#include "potf2_blocked.cuh"
 
 namespace {
 
@@ -35,120 +36,8 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 }
 
 
-// =================================================================================================
-// k_potf2: unblocked Cholesky of one nb x nb (nb <= 64) diagonal block per chain.  256 threads as a
-// 16 x 16 grid, thread (ty,tx) keeps the 4x4 sub-block rows 4ty.., cols 4tx.. in registers.  Step k
-// broadcasts column k through shared memory (double buffered: one barrier per step) and applies
-// the rank-1 update A[i][j] -= A[i][k] A[j][k] / d_k; columns are scaled by 1/sqrt(d_k) at the end.
-// A non-positive (or NaN) pivot d_k records info = 1-based global row (first failure wins).
-// =================================================================================================
-__global__ void __launch_bounds__(256) k_potf2(double* __restrict__ A_all, int64_t ld, int64_t stride, int j0, int nloc,
-                                               int32_t* __restrict__ info, double* __restrict__ Winv)
-{
-    __shared__ double s_col[2][64];
-    __shared__ double s_d[64];
-    __shared__ __align__(16) double s_Lt[64][66];   // s_Lt[j][i] = L[i][j] (column j of L contiguous in i), for the inverse
-    const int c = blockIdx.x;
-    double* A = A_all + (size_t)c * stride + (size_t)j0 * ld + j0;
-    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
-    const bool active = ty >= tx;
-    double a[4][4];
-#pragma unroll
-    for (int rr = 0; rr < 4; ++rr)
-#pragma unroll
-        for (int cc = 0; cc < 4; ++cc) {
-            const int i = 4 * ty + rr, j = 4 * tx + cc;
-            double val = (i == j) ? 1.0 : 0.0;                    // identity padding for a ragged block
-            if (active && i < nloc && j <= i) val = A[(size_t)i * ld + j];
-            a[rr][cc] = val;
-        }
-    int fail_row = 0;
-    for (int k = 0; k < nloc; ++k) {
-        const int buf = k & 1;
-        if (tx == (k >> 2) && active) {
-            const int kc = k & 3;
-#pragma unroll
-            for (int rr = 0; rr < 4; ++rr) {
-                double val = a[rr][0];
-                if (kc == 1) val = a[rr][1];
-                if (kc == 2) val = a[rr][2];
-                if (kc == 3) val = a[rr][3];
-                s_col[buf][4 * ty + rr] = val;
-            }
-        }
-        __syncthreads();
-        const double d = s_col[buf][k];
-        if (!(d > 0.0) && fail_row == 0) fail_row = j0 + k + 1;
-        if (threadIdx.x == 0) s_d[k] = d;
-        if (active && 4 * ty + 3 > k) {
-            const double invd = 1.0 / d;
-            double li[4], lj[4];
-#pragma unroll
-            for (int rr = 0; rr < 4; ++rr) li[rr] = s_col[buf][4 * ty + rr] * invd;
-#pragma unroll
-            for (int cc = 0; cc < 4; ++cc) lj[cc] = s_col[buf][4 * tx + cc];
-#pragma unroll
-            for (int rr = 0; rr < 4; ++rr)
-#pragma unroll
-                for (int cc = 0; cc < 4; ++cc)
-                    if (4 * tx + cc > k) a[rr][cc] -= li[rr] * lj[cc];
-        }
-    }
-    __syncthreads();
-    if (threadIdx.x == 0 && fail_row != 0 && info != nullptr && info[c] == 0) info[c] = fail_row;
-    if (active) {
-#pragma unroll
-        for (int cc = 0; cc < 4; ++cc) {
-            const int j = 4 * tx + cc;
-            if (j >= nloc) continue;
-            const double piv = sqrt(s_d[j]);
-            const double inv = 1.0 / piv;
-#pragma unroll
-            for (int rr = 0; rr < 4; ++rr) {
-                const int i = 4 * ty + rr;
-                const double lv = (i == j) ? piv : a[rr][cc] * inv;
-                if (i < nloc && j <= i) A[(size_t)i * ld + j] = lv;
-                if (j <= i) s_Lt[j][i] = lv;
-            }
-        }
-    }
-    // W = L^-1 (lower), needed by the tensor-core triangular solve of the rows below (k_trsm): thread j
-    // forward-substitutes column j, right-looking so that every FMA of a step is independent; the
-    // column of L it needs at step i is a broadcast 16-byte shared-memory read.  Only full blocks
-    // have rows below them.
-    if (Winv == nullptr || nloc < 64) return;
-    __syncthreads();
-    if (threadIdx.x < 64) {
-        const int j = threadIdx.x;
-        double r[64];
-#pragma unroll
-        for (int i = 0; i < 64; ++i) r[i] = (i == j) ? 1.0 : 0.0;
-#pragma unroll
-        for (int i = 0; i < 64; ++i) {
-            const double wi = r[i] * rsqrt(s_d[i]);
-            r[i] = wi;
-            if (i & 1) {
-#pragma unroll
-                for (int m = i + 1; m < 64; m += 2) {
-                    const double2 l2 = *reinterpret_cast<const double2*>(&s_Lt[i][m]);
-                    r[m] -= l2.x * wi;
-                    r[m + 1] -= l2.y * wi;
-                }
-            } else {
-                r[i + 1] -= s_Lt[i][i + 1] * wi;
-#pragma unroll
-                for (int m = i + 2; m < 64; m += 2) {
-                    const double2 l2 = *reinterpret_cast<const double2*>(&s_Lt[i][m]);
-                    r[m] -= l2.x * wi;
-                    r[m + 1] -= l2.y * wi;
-                }
-            }
-        }
-        double* W = Winv + (size_t)c * 64 * 64;
-#pragma unroll
-        for (int i = 0; i < 64; ++i) W[i * 64 + j] = r[i];          // W[i][j], coalesced across the 64 threads
-    }
-}
+// k_potf2 (diagonal blocks): potf2_blocked.cuh
+using potf2::k_potf2;
 
 // =================================================================================================
 // k_trsm: rows gi in [r_lo, r_hi) of the panel at columns [j0, j0+64): X L^T = A  <=>  X = A W^T with
@@ -469,6 +358,7 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
     if (!attr_set) {
         BD_CUDA(ctx, cudaFuncSetAttribute(k_syrk, cudaFuncAttributeMaxDynamicSharedMemorySize, SYRK_SMEM));
         BD_CUDA(ctx, cudaFuncSetAttribute(k_trsm, cudaFuncAttributeMaxDynamicSharedMemorySize, trsm_smem));
+        BD_CUDA(ctx, cudaFuncSetAttribute(k_potf2, cudaFuncAttributeMaxDynamicSharedMemorySize, potf2::SMEM_BYTES));
         attr_set = true;
     }
     const int n = ctx->M, C = ctx->C;
@@ -489,7 +379,7 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
         {
             if (J1 - J0 <= BD_NB_INNER) {
                 const int nloc = J1 - J0;
-                BD_LAUNCH(ctx, k_potf2, dim3(C), dim3(256), 0, A, ld, stride, J0, nloc, info, ctx->Winv);
+                BD_LAUNCH(ctx, k_potf2, dim3(C), dim3(256), potf2::SMEM_BYTES, A, ld, stride, J0, nloc, info, ctx->Winv);
                 if (J1 < n)
                     BD_LAUNCH(ctx, k_trsm, dim3((n - J1 + TRSM_ROWS - 1) / TRSM_ROWS, C), dim3(256), trsm_smem, A, ld, stride, J0,
                               J1, n, ctx->Winv);
