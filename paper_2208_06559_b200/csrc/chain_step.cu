@@ -41,7 +41,12 @@ constexpr int CS_THREADS = 256;
 constexpr int CS_WARPS = 8;
 constexpr int CS_MTW = 5;                 // m-tiles per warp  -> M <= 8*8*5 = 320
 constexpr int CS_MAXM = 8 * CS_WARPS * CS_MTW;
-constexpr int CS_STAGES = 4;              // operand ring depth (k-groups in flight)
+#ifndef CS_KG_N
+#define CS_KG_N 2
+#define CS_STAGES_N 2
+#endif
+constexpr int CS_KG = CS_KG_N;            // k-groups per ring stage: one mbarrier round trip (~90 cycles) per CS_KG k-groups
+constexpr int CS_STAGES = CS_STAGES_N;    // ring stages
 
 struct ChainStepParams {
     int N, C;
@@ -124,8 +129,9 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
 
     extern __shared__ __align__(128) double sm[];
     const int slot_d = (max(MP - NBP, NBP) * 4 + 15) & ~15;     // ring slot: rows k0..MP-1 of one k-group, k0 >= NBP
-    double* ring = sm;                                          // [CS_STAGES][slot_d]   operand ring (TMA destination)
-    double* tile = ring + CS_STAGES * slot_d;                   // [NQP][MP+1][4]  panel block column, fragment-major
+    const int slot_s = CS_KG * slot_d;                          // one ring stage = CS_KG k-groups
+    double* ring = sm;                                          // [CS_STAGES][CS_KG][slot_d]   operand ring (TMA destination)
+    double* tile = ring + CS_STAGES * slot_s;                   // [NQP][MP+1][4]  panel block column, fragment-major
     double* winv = tile + (size_t)NQP * MT4;                    // [NBP][WS] inverse of the diagonal block
     double* sR = winv + NBP * WS;                               // [MP] positions
     double* sF = sR + MP;                                       // [MP] bead forces (later: unshifted new positions)
@@ -196,13 +202,21 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                 const int nq = k0 >> 2;
                 const uint32_t stage_bytes = (uint32_t)(MP - k0) * 32u;
                 // operand ring prologue: the first CS_STAGES-1 k-groups of this panel (thread 0 = producer)
+                // k-groups per ring stage: as many as fit into a stage (sized for CS_KG k-groups of the longest panel) and
+                // divide nq (a multiple of 6) -- one mbarrier round trip (~90 cycles) then covers 2, 3 or 6 k-groups
+                const int sub_d = (MP - k0) * 4;                // doubles of one k-group (rows k0 .. MP-1)
+                const int kg = (6 * sub_d <= slot_s) ? 6 : (3 * sub_d <= slot_s) ? 3 : CS_KG;
+                const int nqs = nq / kg;                        // stages of this panel
+                auto produce = [&](int qs, uint32_t Gs) {       // thread 0: stage qs of this panel -> ring slot Gs % S
+                    const uint32_t sl = Gs % CS_STAGES;
+                    if (Gs >= CS_STAGES) mbar_wait(bar_empty + 8 * sl, ((Gs / CS_STAGES) - 1) & 1);
+                    mbar_expect_tx(bar_full + 8 * sl, kg * stage_bytes);
+                    for (int h = 0; h < kg; ++h)
+                        tma_bulk_g2s(ring_u32 + (sl * slot_s + h * sub_d) * 8, Lg + ((size_t)(qs * kg + h) * MP + k0) * 4, stage_bytes,
+                                     bar_full + 8 * sl);
+                };
                 if (tid == 0) {
-                    for (int q = 0; q < CS_STAGES - 1 && q < nq; ++q) {
-                        const uint32_t G_ = git + q, sl = G_ % CS_STAGES;
-                        if (G_ >= CS_STAGES) mbar_wait(bar_empty + 8 * sl, ((G_ / CS_STAGES) - 1) & 1);
-                        mbar_expect_tx(bar_full + 8 * sl, stage_bytes);
-                        tma_bulk_g2s(ring_u32 + sl * slot_d * 8, Lg + ((size_t)q * MP + k0) * 4, stage_bytes, bar_full + 8 * sl);
-                    }
+                    for (int q = 0; q < CS_STAGES - 1 && q < nqs; ++q) produce(q, git + q);
                 }
                 // (a) block column of D: pairs (row bead jb0+ib, panel bead jb0+jb)
                 for (int p = tid; p < nrb * PB; p += CS_THREADS) {
@@ -253,32 +267,29 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                     const int b_off = g * 4 + t;                               // + nt*32
                     auto gemm = [&](auto i0c) {
                         constexpr int I0 = decltype(i0c)::value;
-                        for (int q = 0; q < nq; ++q) {
+                        for (int q = 0; q < nqs; ++q) {
                             const uint32_t G_ = git + q, sl = G_ % CS_STAGES;
                             mbar_wait(bar_full + 8 * sl, (G_ / CS_STAGES) & 1);
-                            const double* st = ring + (size_t)sl * slot_d;
+                            // refill first (stage q + S - 1 goes where stage q - 1 was): the copy flies during this stage's DMMAs
+                            if (tid == 0 && q + CS_STAGES - 1 < nqs) produce(q + CS_STAGES - 1, G_ + CS_STAGES - 1);
                             if constexpr (I0 < CS_MTW) {
-                                double af[CS_MTW], bf[NT];
+                                for (int h = 0; h < kg; ++h) {
+                                    const double* st = ring + (size_t)sl * slot_s + h * sub_d;
+                                    double af[CS_MTW], bf[NT];
 #pragma unroll
-                                for (int nt = 0; nt < NT; ++nt) bf[nt] = st[b_off + nt * 32];
+                                    for (int nt = 0; nt < NT; ++nt) bf[nt] = st[b_off + nt * 32];
 #pragma unroll
-                                for (int i = I0; i < CS_MTW; ++i) af[i] = (i + 1 < CS_MTW || act[i]) ? st[a_off + i * (8 * CS_WARPS * 4)] : 0.0;
+                                    for (int i = I0; i < CS_MTW; ++i) af[i] = (i + 1 < CS_MTW || act[i]) ? st[a_off + i * (8 * CS_WARPS * 4)] : 0.0;
 #pragma unroll
-                                for (int i = I0; i < CS_MTW; ++i) {
-                                    if (i + 1 == CS_MTW && !act[i]) continue;      // only the last slot can lie beyond nmt
+                                    for (int i = I0; i < CS_MTW; ++i) {
+                                        if (i + 1 == CS_MTW && !act[i]) continue;  // only the last slot can lie beyond nmt
 #pragma unroll
-                                    for (int nt = 0; nt < NT; ++nt) dmma(acc[i][nt][0], acc[i][nt][1], af[i], bf[nt]);
+                                        for (int nt = 0; nt < NT; ++nt) dmma(acc[i][nt][0], acc[i][nt][1], af[i], bf[nt]);
+                                    }
                                 }
                             }
                             __syncwarp();
                             if (lane == 0) mbar_arrive(bar_empty + 8 * sl);    // this warp is done with the slot
-                            if (tid == 0 && q + CS_STAGES - 1 < nq) {          // refill: k-group q + S - 1
-                                const uint32_t Gn = G_ + CS_STAGES - 1, sn = Gn % CS_STAGES;
-                                if (Gn >= CS_STAGES) mbar_wait(bar_empty + 8 * sn, ((Gn / CS_STAGES) - 1) & 1);
-                                mbar_expect_tx(bar_full + 8 * sn, stage_bytes);
-                                tma_bulk_g2s(ring_u32 + sn * slot_d * 8, Lg + ((size_t)(q + CS_STAGES - 1) * MP + k0) * 4, stage_bytes,
-                                             bar_full + 8 * sn);
-                            }
                         }
                     };
                     int imin = 0;
@@ -290,29 +301,25 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                     if (imin < CS_MTW && !act[imin]) imin = CS_MTW;
                     if (imin < CS_MTW - 1 && !act[CS_MTW - 2]) {
                         // short chain: fewer than CS_MTW-1 slots in use -> generic predicated path is cheap enough
-                        for (int q = 0; q < nq; ++q) {
+                        for (int q = 0; q < nqs; ++q) {
                             const uint32_t G_ = git + q, sl = G_ % CS_STAGES;
                             mbar_wait(bar_full + 8 * sl, (G_ / CS_STAGES) & 1);
-                            const double* st = ring + (size_t)sl * slot_d;
-                            double bf[NT];
+                            if (tid == 0 && q + CS_STAGES - 1 < nqs) produce(q + CS_STAGES - 1, G_ + CS_STAGES - 1);
+                            for (int h = 0; h < kg; ++h) {
+                                const double* st = ring + (size_t)sl * slot_s + h * sub_d;
+                                double bf[NT];
 #pragma unroll
-                            for (int nt = 0; nt < NT; ++nt) bf[nt] = st[b_off + nt * 32];
+                                for (int nt = 0; nt < NT; ++nt) bf[nt] = st[b_off + nt * 32];
 #pragma unroll
-                            for (int i = 0; i < CS_MTW; ++i) {
-                                if (!act[i]) continue;
-                                const double af = st[a_off + i * (8 * CS_WARPS * 4)];
+                                for (int i = 0; i < CS_MTW; ++i) {
+                                    if (!act[i]) continue;
+                                    const double af = st[a_off + i * (8 * CS_WARPS * 4)];
 #pragma unroll
-                                for (int nt = 0; nt < NT; ++nt) dmma(acc[i][nt][0], acc[i][nt][1], af, bf[nt]);
+                                    for (int nt = 0; nt < NT; ++nt) dmma(acc[i][nt][0], acc[i][nt][1], af, bf[nt]);
+                                }
                             }
                             __syncwarp();
                             if (lane == 0) mbar_arrive(bar_empty + 8 * sl);
-                            if (tid == 0 && q + CS_STAGES - 1 < nq) {
-                                const uint32_t Gn = G_ + CS_STAGES - 1, sn = Gn % CS_STAGES;
-                                if (Gn >= CS_STAGES) mbar_wait(bar_empty + 8 * sn, ((Gn / CS_STAGES) - 1) & 1);
-                                mbar_expect_tx(bar_full + 8 * sn, stage_bytes);
-                                tma_bulk_g2s(ring_u32 + sn * slot_d * 8, Lg + ((size_t)(q + CS_STAGES - 1) * MP + k0) * 4, stage_bytes,
-                                             bar_full + 8 * sn);
-                            }
                         }
                     } else {
                         switch (imin) {
@@ -324,7 +331,7 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                             default: gemm(std::integral_constant<int, CS_MTW>{}); break;
                         }
                     }
-                    git += (uint32_t)nq;
+                    git += (uint32_t)nqs;
                 }
 #pragma unroll
                 for (int i = 0; i < CS_MTW; ++i)
@@ -502,7 +509,7 @@ size_t chain_step_smem(int M)
 {
     const int NBP = 8 * NT, MP = (M + 7) & ~7;
     const size_t slot_d = ((size_t)(MP - NBP > NBP ? MP - NBP : NBP) * 4 + 15) & ~(size_t)15;
-    return sizeof(double) * (CS_STAGES * slot_d + (size_t)(NBP / 4) * (MP + 1) * 4 + (size_t)NBP * (NBP + 4) + 4 * (size_t)MP +
+    return sizeof(double) * (CS_STAGES * CS_KG * slot_d + (size_t)(NBP / 4) * (MP + 1) * 4 + (size_t)NBP * (NBP + 4) + 4 * (size_t)MP +
                              (MP + NBP) + 64 + 96 + 32);
 }
 
