@@ -366,13 +366,13 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                     }
                     const bool row_ok = lane < nrows;
                     __syncwarp();
-                    const int f = warp_chol<NBP, 8>(x, lane, sCol, sRinv, 1, [&](int k, double l) {
+                    const int f = warp_chol<NBP, 4>(x, lane, sCol, sRinv, 1, [&](int k, double l) {
                         if (row_ok) tile[TIDX(lane, k)] = (lane >= k) ? l : 0.0;
                     });
                     if (lane == 0 && f != 0 && sFail == 0) sFail = k0 + f;
                 } else if (warp == 1) {
-                    // W = L_kk^-1 (-> winv) by forward substitution, 8 pivots behind warp 0 (named barriers 1..3)
-                    warp_inverse<NBP, 8, WS>(lane, nrows, sRinv, winv, 1, [&](int k, int j) { return tile[TIDX(k, j)]; });
+                    // W = L_kk^-1 (-> winv) by forward substitution, 4 pivots behind warp 0 (named barriers 1..6)
+                    warp_inverse<NBP, 4, WS>(lane, nrows, sRinv, winv, 1, [&](int k, int j) { return tile[TIDX(k, j)]; });
                 } else {
                     const int npan = (M + NBP - 1) / NBP, bps = (Nb + npan - 1) / npan;
                     const int ib0 = (k0 / NBP) * bps, ib1 = min(ib0 + bps, Nb);
