@@ -4,7 +4,7 @@
 // The block is split 32 + 32:   A = [A11 . ; A21 A22]
 //   1. L11 = chol(A11) by warp 0 (one row per lane, registers + shuffles, warp_chol.cuh) while warp 1 forms
 //      W11 = L11^-1 by forward substitution 8 pivots behind it
-//   2. L21 = A21 W11^T                      (all 256 threads, 4 outputs each, operands in shared memory)
+//   2. L21 = A21 W11^T                      (8 warps, DMMA m8n8k4, operands in shared memory)
 //   3. A22 -= L21 L21^T
 //   4. L22 = chol(A22), W22 = L22^-1        (as step 1)
 //   5. W21 = -W22 (L21 W11)
@@ -20,18 +20,26 @@ namespace potf2 {
 constexpr int HB = 32;            // half block
 constexpr int SLDP = 65;          // row stride of the 64 x 64 working copies (odd: conflict-free columns)
 
-// out[c] = sum_p X[i][p] * Y(j, p), j = jq + c, c = 0..3: product of two 32 x 32 operands held in shared memory;
+// out = sum_p X[i][p] * Y(j, p): product of two 32 x 32 operands held in shared memory on the FP64 tensor cores.
+// Warp w owns output rows 8 (w & 3) .. +7 and columns 16 (w >> 2) .. +15 (two m8n8k4 accumulators, 8 k-steps);
 // yt selects Y(j, p) = Y[p][j] (plain product X Y) or Y[j][p] (X Y^T).  Triangular operands carry explicit zeros.
-__device__ __forceinline__ void gemm32(const double* __restrict__ X, const double* __restrict__ Y, bool yt, int i, int jq,
-                                       double (&out)[4])
+// Lane (g, t) ends up with out[nn][0..1] = element (row 8 (w & 3) + g, column 16 (w >> 2) + 8 nn + 2 t + {0, 1}).
+__device__ __forceinline__ void gemm32(const double* __restrict__ X, const double* __restrict__ Y, bool yt, int warp, int lane,
+                                       double (&out)[2][2])
 {
+    const int g = lane >> 2, t = lane & 3, mt = warp & 3, nt0 = (warp >> 2) * 2;
+    out[0][0] = out[0][1] = out[1][0] = out[1][1] = 0.0;
 #pragma unroll
-    for (int c = 0; c < 4; ++c) out[c] = 0.0;
-#pragma unroll 8
-    for (int p = 0; p < HB; ++p) {
-        const double x = X[i * SLDP + p];
+    for (int ks = 0; ks < HB / 4; ++ks) {
+        const double a = X[(8 * mt + g) * SLDP + 4 * ks + t];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) out[c] = fma(x, yt ? Y[p * SLDP + jq + c] : Y[(jq + c) * SLDP + p], out[c]);
+        for (int nn = 0; nn < 2; ++nn) {
+            const int j = 8 * (nt0 + nn) + g, p = 4 * ks + t;
+            const double b = yt ? Y[p * SLDP + j] : Y[j * SLDP + p];
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                         : "+d"(out[nn][0]), "+d"(out[nn][1])
+                         : "d"(a), "d"(b));
+        }
     }
 }
 
@@ -72,32 +80,40 @@ __global__ void __launch_bounds__(256) k_potf2(double* __restrict__ A_all, int64
             warp_inverse<HB, 8, SLDP>(lane, HB, sRinv + o, Wm + o * SLDP + o, 1, [&](int k, int j) { return S[(o + k) * SLDP + o + j]; });
         }
     };
-    const int i = tid >> 3, jq = (tid & 7) * 4;
-    double out[4];
+    const int oi = 8 * (warp & 3) + (lane >> 2), oj = 16 * (warp >> 2) + 2 * (lane & 3);   // this lane's outputs: (oi, oj + 8 nn + {0, 1})
+    double out[2][2];
 
     factor_half(0);
     __syncthreads();
     if (nloc > HB) {
-        gemm32(S + HB * SLDP, Wm, false, i, jq, out);              // L21 = A21 W11^T
+        gemm32(S + HB * SLDP, Wm, false, warp, lane, out);         // L21 = A21 W11^T
         __syncthreads();
 #pragma unroll
-        for (int q = 0; q < 4; ++q) S[(HB + i) * SLDP + jq + q] = out[q];
-        __syncthreads();
-        gemm32(S + HB * SLDP, S + HB * SLDP, false, i, jq, out);   // A22 -= L21 L21^T (lower part)
+        for (int nn = 0; nn < 2; ++nn)
 #pragma unroll
-        for (int q = 0; q < 4; ++q)
-            if (jq + q <= i) S[(HB + i) * SLDP + HB + jq + q] -= out[q];
+            for (int e = 0; e < 2; ++e) S[(HB + oi) * SLDP + oj + 8 * nn + e] = out[nn][e];
+        __syncthreads();
+        gemm32(S + HB * SLDP, S + HB * SLDP, false, warp, lane, out);   // A22 -= L21 L21^T (lower part)
+#pragma unroll
+        for (int nn = 0; nn < 2; ++nn)
+#pragma unroll
+            for (int e = 0; e < 2; ++e)
+                if (oj + 8 * nn + e <= oi) S[(HB + oi) * SLDP + HB + oj + 8 * nn + e] -= out[nn][e];
         __syncthreads();
         factor_half(HB);
         __syncthreads();
-        gemm32(S + HB * SLDP, Wm, true, i, jq, out);               // T = L21 W11 -> the (still empty) W21 area
+        gemm32(S + HB * SLDP, Wm, true, warp, lane, out);          // T = L21 W11 -> the (still empty) W21 area
 #pragma unroll
-        for (int q = 0; q < 4; ++q) Wm[(HB + i) * SLDP + jq + q] = out[q];
+        for (int nn = 0; nn < 2; ++nn)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) Wm[(HB + oi) * SLDP + oj + 8 * nn + e] = out[nn][e];
         __syncthreads();
-        gemm32(Wm + HB * SLDP + HB, Wm + HB * SLDP, true, i, jq, out);   // W21 = -W22 T
+        gemm32(Wm + HB * SLDP + HB, Wm + HB * SLDP, true, warp, lane, out);   // W21 = -W22 T
         __syncthreads();
 #pragma unroll
-        for (int q = 0; q < 4; ++q) Wm[(HB + i) * SLDP + jq + q] = -out[q];
+        for (int nn = 0; nn < 2; ++nn)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) Wm[(HB + oi) * SLDP + oj + 8 * nn + e] = -out[nn][e];
         __syncthreads();
     }
     if (tid == 0 && sFail != 0 && info != nullptr && info[c] == 0) info[c] = sFail;
