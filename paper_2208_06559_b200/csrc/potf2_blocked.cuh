@@ -43,6 +43,27 @@ __device__ __forceinline__ void gemm32(const double* __restrict__ X, const doubl
     }
 }
 
+// rows / columns o .. o+31 of the working copy: warp 0 factors (L back into S, 1 / L_kk into s_rinv), warp 1 forms the
+// inverse of that 32 x 32 factor in Wm, 8 pivots behind (named barriers 1..4).  Must be inlined at both call sites:
+// out of line, the per-lane row arrays land in local memory (measured: 29 k instead of 7 k cycles).
+__device__ __forceinline__ void factor_half(double* __restrict__ S, double* __restrict__ Wm, double* __restrict__ sCol,
+                                            double* __restrict__ sRinv, const int o, const int lane, const int warp, const int j0,
+                                            int* sFail)
+{
+    if (warp == 0) {
+        double x[HB];
+#pragma unroll
+        for (int j = 0; j < HB; ++j) x[j] = S[(o + max(lane, j)) * SLDP + o + min(lane, j)];
+        __syncwarp();
+        const int f = warp_chol<HB, 8>(x, lane, sCol, sRinv + o, 1, [&](int k, double l) {
+            S[(o + lane) * SLDP + o + k] = (lane >= k) ? l : 0.0;
+        });
+        if (lane == 0 && f != 0 && *sFail == 0) *sFail = j0 + o + f;
+    } else if (warp == 1) {
+        warp_inverse<HB, 8, SLDP>(lane, HB, sRinv + o, Wm + o * SLDP + o, 1, [&](int k, int j) { return S[(o + k) * SLDP + o + j]; });
+    }
+}
+
 constexpr int SMEM_BYTES = (2 * 64 * SLDP + 128) * (int)sizeof(double);
 
 __global__ void __launch_bounds__(256) k_potf2(double* __restrict__ A_all, int64_t ld, int64_t stride, int j0, int nloc,
@@ -56,52 +77,53 @@ __global__ void __launch_bounds__(256) k_potf2(double* __restrict__ A_all, int64
     __shared__ int sFail;
     const int c = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     double* A = A_all + (size_t)c * stride + (size_t)j0 * ld + j0;
-    for (int idx = tid; idx < 64 * 64; idx += 256) {
-        const int i = idx >> 6, j = idx & 63;
-        double v = (i == j) ? 1.0 : 0.0;                           // identity padding for a ragged block
-        if (i < nloc && j <= i) v = A[(size_t)i * ld + j];
-        S[i * SLDP + j] = (j <= i) ? v : 0.0;
-        Wm[i * SLDP + j] = 0.0;
+    {
+        double v[16];                                              // all 16 loads of a thread in flight at once
+#pragma unroll
+        for (int it = 0; it < 16; ++it) {
+            const int idx = tid + 256 * it, i = idx >> 6, j = idx & 63;
+            v[it] = (i == j) ? 1.0 : 0.0;                          // identity padding for a ragged block
+            if (i < nloc && j <= i) v[it] = A[(size_t)i * ld + j];
+        }
+#pragma unroll
+        for (int it = 0; it < 16; ++it) {
+            const int idx = tid + 256 * it, i = idx >> 6, j = idx & 63;
+            S[i * SLDP + j] = (j <= i) ? v[it] : 0.0;
+            Wm[i * SLDP + j] = 0.0;
+        }
     }
     if (tid == 0) sFail = 0;
     __syncthreads();
 
-    auto factor_half = [&](int o) {                                // rows / columns o .. o+31
-        if (warp == 0) {
-            double x[HB];
-#pragma unroll
-            for (int j = 0; j < HB; ++j) x[j] = S[(o + max(lane, j)) * SLDP + o + min(lane, j)];
-            __syncwarp();
-            const int f = warp_chol<HB, 8>(x, lane, sCol, sRinv + o, 1, [&](int k, double l) {
-                S[(o + lane) * SLDP + o + k] = (lane >= k) ? l : 0.0;
-            });
-            if (lane == 0 && f != 0 && sFail == 0) sFail = j0 + o + f;
-        } else if (warp == 1) {
-            warp_inverse<HB, 8, SLDP>(lane, HB, sRinv + o, Wm + o * SLDP + o, 1, [&](int k, int j) { return S[(o + k) * SLDP + o + j]; });
-        }
-    };
     const int oi = 8 * (warp & 3) + (lane >> 2), oj = 16 * (warp >> 2) + 2 * (lane & 3);   // this lane's outputs: (oi, oj + 8 nn + {0, 1})
     double out[2][2];
 
-    factor_half(0);
-    __syncthreads();
-    if (nloc > HB) {
-        gemm32(S + HB * SLDP, Wm, false, warp, lane, out);         // L21 = A21 W11^T
+    // ONE copy of the factor / inverse code, run once per half: a second inlined copy (64 KB further into the kernel)
+    // ran 4x slower than the first one (22 k against 5.5 k cycles for the same 32 pivots -- instruction fetch of
+    // ~1700 straight-line instructions that are cold at every launch), a loop re-runs warm instructions.
+    const int nh = (nloc > HB) ? 2 : 1;
+#pragma unroll 1
+    for (int hh = 0; hh < nh; ++hh) {
+        factor_half(S, Wm, sCol, sRinv, hh * HB, lane, warp, j0, &sFail);
         __syncthreads();
+        if (hh == 0 && nh == 2) {
+            gemm32(S + HB * SLDP, Wm, false, warp, lane, out);         // L21 = A21 W11^T
+            __syncthreads();
 #pragma unroll
-        for (int nn = 0; nn < 2; ++nn)
+            for (int nn = 0; nn < 2; ++nn)
 #pragma unroll
-            for (int e = 0; e < 2; ++e) S[(HB + oi) * SLDP + oj + 8 * nn + e] = out[nn][e];
-        __syncthreads();
-        gemm32(S + HB * SLDP, S + HB * SLDP, false, warp, lane, out);   // A22 -= L21 L21^T (lower part)
+                for (int e = 0; e < 2; ++e) S[(HB + oi) * SLDP + oj + 8 * nn + e] = out[nn][e];
+            __syncthreads();
+            gemm32(S + HB * SLDP, S + HB * SLDP, false, warp, lane, out);   // A22 -= L21 L21^T (lower part)
 #pragma unroll
-        for (int nn = 0; nn < 2; ++nn)
+            for (int nn = 0; nn < 2; ++nn)
 #pragma unroll
-            for (int e = 0; e < 2; ++e)
-                if (oj + 8 * nn + e <= oi) S[(HB + oi) * SLDP + HB + oj + 8 * nn + e] -= out[nn][e];
-        __syncthreads();
-        factor_half(HB);
-        __syncthreads();
+                for (int e = 0; e < 2; ++e)
+                    if (oj + 8 * nn + e <= oi) S[(HB + oi) * SLDP + HB + oj + 8 * nn + e] -= out[nn][e];
+            __syncthreads();
+        }
+    }
+    if (nh == 2) {
         gemm32(S + HB * SLDP, Wm, true, warp, lane, out);          // T = L21 W11 -> the (still empty) W21 area
 #pragma unroll
         for (int nn = 0; nn < 2; ++nn)
