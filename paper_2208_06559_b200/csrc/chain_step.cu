@@ -397,6 +397,12 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
 
                 // (d) rows below the panel: X = S W^T (DMMA, zero blocks of W skipped); panel rows: L_kk.
                 //     X -> Lg (fragment-major) and y += X dW.
+                //     The fragments of W are the same for every m-tile of the warp: loaded once per panel.
+                double wf[2 * NT][NT];
+#pragma unroll
+                for (int qq = 0; qq < 2 * NT; ++qq)
+#pragma unroll
+                    for (int nt = 0; nt < NT; ++nt) wf[qq][nt] = (qq <= 2 * nt + 1) ? winv[(8 * nt + g) * WS + 4 * qq + t] : 0.0;
 #pragma unroll
                 for (int i = 0; i < CS_MTW; ++i) {
                     if (!act[i]) continue;
@@ -411,7 +417,7 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                             const double af = tile[qq * MT4 + rr * 4 + t];
 #pragma unroll
                             for (int nt = 0; nt < NT; ++nt)
-                                if (qq <= 2 * nt + 1) dmma(x[nt][0], x[nt][1], af, winv[(8 * nt + g) * WS + 4 * qq + t]);
+                                if (qq <= 2 * nt + 1) dmma(x[nt][0], x[nt][1], af, wf[qq][nt]);
                         }
                     } else {
 #pragma unroll
