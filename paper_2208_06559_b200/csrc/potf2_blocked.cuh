@@ -3,7 +3,7 @@
 //
 // The block is split 32 + 32:   A = [A11 . ; A21 A22]
 //   1. L11 = chol(A11) by warp 0 (one row per lane, registers + shuffles, warp_chol.cuh) while warp 1 forms
-//      W11 = L11^-1 by forward substitution 8 pivots behind it
+//      W11 = L11^-1 by forward substitution 4 pivots behind it
 //   2. L21 = A21 W11^T                      (8 warps, DMMA m8n8k4, operands in shared memory)
 //   3. A22 -= L21 L21^T
 //   4. L22 = chol(A22), W22 = L22^-1        (as step 1)
@@ -44,7 +44,7 @@ __device__ __forceinline__ void gemm32(const double* __restrict__ X, const doubl
 }
 
 // rows / columns o .. o+31 of the working copy: warp 0 factors (L back into S, 1 / L_kk into s_rinv), warp 1 forms the
-// inverse of that 32 x 32 factor in Wm, 8 pivots behind (named barriers 1..4).  Must be inlined at both call sites:
+// inverse of that 32 x 32 factor in Wm, 4 pivots behind (named barriers 1..8).  Must be inlined at both call sites:
 // out of line, the per-lane row arrays land in local memory (measured: 29 k instead of 7 k cycles).
 __device__ __forceinline__ void factor_half(double* __restrict__ S, double* __restrict__ Wm, double* __restrict__ sCol,
                                             double* __restrict__ sRinv, const int o, const int lane, const int warp, const int j0,
@@ -55,12 +55,12 @@ __device__ __forceinline__ void factor_half(double* __restrict__ S, double* __re
 #pragma unroll
         for (int j = 0; j < HB; ++j) x[j] = S[(o + max(lane, j)) * SLDP + o + min(lane, j)];
         __syncwarp();
-        const int f = warp_chol<HB, 8>(x, lane, sCol, sRinv + o, 1, [&](int k, double l) {
+        const int f = warp_chol<HB, 4>(x, lane, sCol, sRinv + o, 1, [&](int k, double l) {
             S[(o + lane) * SLDP + o + k] = (lane >= k) ? l : 0.0;
         });
         if (lane == 0 && f != 0 && *sFail == 0) *sFail = j0 + o + f;
     } else if (warp == 1) {
-        warp_inverse<HB, 8, SLDP>(lane, HB, sRinv + o, Wm + o * SLDP + o, 1, [&](int k, int j) { return S[(o + k) * SLDP + o + j]; });
+        warp_inverse<HB, 4, SLDP>(lane, HB, sRinv + o, Wm + o * SLDP + o, 1, [&](int k, int j) { return S[(o + k) * SLDP + o + j]; });
     }
 }
 
