@@ -33,6 +33,7 @@ struct bd_ctx {
     int32_t path;           // bd_set_path
     cudaError_t last_cuda;
     int num_sms;
+    bool attr_potrf, attr_chain;   // cudaFuncSetAttribute done for this context's device (no process-wide statics)
 };
 
 extern cudaError_t bd_g_last_cuda;   // last CUDA error seen by any libbd call (for bd_strerror)

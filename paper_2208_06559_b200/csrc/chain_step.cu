@@ -528,11 +528,10 @@ bool bdk_chain_step_supported(const bd_ctx* ctx) { return ctx->M <= CS_MAXM; }
 int bdk_chain_step(bd_ctx* ctx, double* r, uint64_t first_step, int n_steps)
 {
     constexpr int NT = 3;
-    static bool attr_set = false;
     const size_t smem = chain_step_smem<NT>(ctx->M);
-    if (!attr_set) {
+    if (!ctx->attr_chain) {
         BD_CUDA(ctx, cudaFuncSetAttribute(k_chain_step<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_set = true;
+        ctx->attr_chain = true;
     }
     int per_sm = 0;
     BD_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_chain_step<NT>, CS_THREADS, smem));

@@ -353,13 +353,12 @@ int launch_syrk(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int lo, int 
 
 int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
 {
-    static bool attr_set = false;
     const int trsm_smem = TRSM_SMEM;
-    if (!attr_set) {
+    if (!ctx->attr_potrf) {
         BD_CUDA(ctx, cudaFuncSetAttribute(k_syrk, cudaFuncAttributeMaxDynamicSharedMemorySize, SYRK_SMEM));
         BD_CUDA(ctx, cudaFuncSetAttribute(k_trsm, cudaFuncAttributeMaxDynamicSharedMemorySize, trsm_smem));
         BD_CUDA(ctx, cudaFuncSetAttribute(k_potf2, cudaFuncAttributeMaxDynamicSharedMemorySize, potf2::SMEM_BYTES));
-        attr_set = true;
+        ctx->attr_potrf = true;
     }
     const int n = ctx->M, C = ctx->C;
     // outer panel width, from sweeps on B200 (profiles/r01_summary.md): with the recursive panel below, wide outer
