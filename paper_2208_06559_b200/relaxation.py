@@ -1,0 +1,82 @@
+"""Relaxation time lambda(N) from equilibrium runs ("fitting the last
+70 % of the auto-correlation function [of the end-to-end vector] to an exponential decay", :303 equilibrium runs with
+dt = 0.001, K* = 1000, expected scaling R_ee, R_g ~ N^0.5 and lambda ~ N^1.5 with HI).
+
+    python -m paper_2208_06559_b200.relaxation [--rods 10 20 40 80] [--chains 1024] [--hstar 0.5 0.0]
+
+Instead of one chain for 100 relaxation times (the paper's single-chain-per-GPU protocol) an ENSEMBLE of independent
+chains is followed for `--window` Rouse times from equilibrium random-walk starts and the normalised correlation
+C(t) = <R(t).R(0)> / <R(0).R(0)> is averaged over the chains.  All time stepping is `bd_step` (many steps per launch);
+torch is used only to read the end-to-end vectors between launches and for the least-squares fit.  This replaces the
+Rouse stand-in lambda_s of workloads.py (reading A12) by measured values.
+"""
+from __future__ import annotations
+
+import argparse
+import math
+
+import numpy as np
+import torch
+
+from .binding import BD, NOBS
+from .workloads import rouse_lambda
+
+
+def measure(n_rods: int, n_chains: int, hstar: float, dt: float, window: float, samples: int, seed: int = 0):
+    lam_r = rouse_lambda(n_rods + 1)
+    total_steps = int(window * lam_r / dt)
+    stride = max(1, total_steps // samples)
+    bd = BD(n_rods=n_rods, n_chains=n_chains, dt=dt, hstar=hstar, seed=seed)       # K* = 1/dt, a = h* b (or a = b/2 if h* = 0)
+    bd.set_workspace()
+    r = bd.init_random_walk(4242)
+    R0 = (r[:, -1, :] - r[:, 0, :]).clone()
+    norm = float((R0 * R0).sum(dim=1).mean())
+    t, acf = [0.0], [1.0]
+    step = 0
+    for _ in range(samples):
+        bd.step(r, first_step=step, n_steps=stride)
+        step += stride
+        R = r[:, -1, :] - r[:, 0, :]
+        t.append(step * dt)
+        acf.append(float((R * R0).sum(dim=1).mean()) / norm)
+    per, _ = bd.observables(r)
+    torch.cuda.synchronize()
+    assert bd.last_info() == (0, -1)
+    per = per.cpu().numpy()
+    t, acf = np.array(t), np.array(acf)
+    lo = int(0.3 * len(t))                                   # last 70 % of the recorded window
+    ok = acf[lo:] > 0.0
+    slope, _ = np.polyfit(t[lo:][ok], np.log(acf[lo:][ok]), 1)
+    return {"N": n_rods, "hstar": hstar, "lambda": -1.0 / slope, "lambda_rouse": lam_r, "Ree": math.sqrt(per[:, 0].mean()),
+            "Rg": math.sqrt(per[:, 4].mean()), "steps": step, "acf_end": float(acf[-1])}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--rods", type=int, nargs="+", default=[10, 20, 40, 80])
+    ap.add_argument("--chains", type=int, default=1024)
+    ap.add_argument("--hstar", type=float, nargs="+", default=[0.5, 0.0])
+    ap.add_argument("--dt", type=float, default=1e-3)
+    ap.add_argument("--window", type=float, default=2.0, help="length of the run in Rouse relaxation times")
+    ap.add_argument("--samples", type=int, default=200)
+    args = ap.parse_args()
+    print("| h* | N rods | steps | lambda (fit) | Rouse stand-in | R_ee | R_g | C(t_end) |")
+    print("|---|---|---|---|---|---|---|---|")
+    rows = []
+    for h in args.hstar:
+        for n in args.rods:
+            row = measure(n, args.chains, h, args.dt, args.window, args.samples)
+            rows.append(row)
+            print(f"| {h} | {n} | {row['steps']} | {row['lambda']:.4g} | {row['lambda_rouse']:.4g} | {row['Ree']:.4g} | {row['Rg']:.4g} | "
+                  f"{row['acf_end']:.3f} |", flush=True)
+    for h in args.hstar:
+        sel = [r for r in rows if r["hstar"] == h]
+        if len(sel) >= 2:
+            ln = np.log([r["N"] for r in sel])
+            for key in ("lambda", "Ree", "Rg"):
+                e = np.polyfit(ln, np.log([r[key] for r in sel]), 1)[0]
+                print(f"h* = {h}: {key} ~ N^{e:.2f}")
+
+
+if __name__ == "__main__":
+    main()
