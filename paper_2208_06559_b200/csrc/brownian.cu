@@ -65,15 +65,22 @@ __global__ void __launch_bounds__(kTrmvWarps * 32) k_trmv(int M, const double* _
     if (lane == 0) y_all[(size_t)c * M + row] = s;
 }
 
-// Variant for LONG chains (M > TRMV_STAGED_MIN_M).  A CTA takes a block of 32 adjacent rows, four rows per warp; the
-// blocks with the longest rows are scheduled first.  dW is staged through shared
-// memory in chunks of TRMV_CHUNK columns, double buffered, and re-used by all rows of the CTA: at M = 30003 the
-// vector (240 KB) no longer fits in L1 and the first version (one row per warp, dW from global memory) fetched as
-// many bytes of dW from L2 as of L from HBM (4.27 TB/s at c5 against 5.1 TB/s at c4; this variant: 4.58 TB/s at c5, but
-// 4.5 TB/s at c3/c4 where the one-row-per-warp kernel is faster -- the barrier per chunk costs more than L1 misses there).  Lanes read 16-byte pairs of
-// four rows: 8 independent 16-byte loads in flight per lane.
-constexpr int TRMV_STAGED_MIN_M = 16384;   // dW of 128 KB still lives in L1 beside the row streams
-constexpr int TRMV_WARPS = 8, TRMV_RPW = 4, TRMV_BLK = TRMV_WARPS * TRMV_RPW, TRMV_CHUNK = 2048;
+// Variant for M > TRMV_STAGED_MIN_M.  A CTA takes a block of 16 adjacent rows, two rows per warp; the blocks with the
+// longest rows are scheduled first.  dW is staged through shared memory in chunks of TRMV_CHUNK columns, double
+// buffered, and re-used by all rows of the CTA: at M = 30003 the vector (240 KB) no longer fits in L1 and the
+// one-row-per-warp kernel fetched as many bytes of dW from L2 as of L from HBM.  Measured on B200 (GB/s at c3 / c4 / c5,
+// HBM copy peak 6553): one row per warp 4945 / 5073 / 4265; this kernel with 4 rows per warp 4500 / 4540 / 4560, with
+// 1 row per warp - / 5524 / 5995, with 2 rows per warp 5186 / 5454 / 6042 (fewer rows per CTA = a finer tail); pairing a
+// long with a short block per CTA: 4037 at c5 (half the CTAs, half the bytes in flight).  Lanes read 16-byte pairs.
+#ifndef TRMV_MIN_M_N
+#define TRMV_MIN_M_N 1024
+#endif
+constexpr int TRMV_STAGED_MIN_M = TRMV_MIN_M_N;   // below: one row per warp, dW through L1
+#ifndef TRMV_RPW_N
+#define TRMV_RPW_N 2
+#define TRMV_CHUNK_N 2048
+#endif
+constexpr int TRMV_WARPS = 8, TRMV_RPW = TRMV_RPW_N, TRMV_BLK = TRMV_WARPS * TRMV_RPW, TRMV_CHUNK = TRMV_CHUNK_N;
 
 __global__ void __launch_bounds__(TRMV_WARPS * 32) k_trmv_staged(int M, const double* __restrict__ L_all, int64_t ld, int64_t stride,
                                                          const double* __restrict__ dW_all, double* __restrict__ y_all)
@@ -99,7 +106,9 @@ __global__ void __launch_bounds__(TRMV_WARPS * 32) k_trmv_staged(int M, const do
         Lr[r] = Lc + (size_t)min(row, M - 1) * ld;
         acc[r] = 0.0;
     }
-    const int nmax = n[TRMV_RPW - 1] > 0 ? n[TRMV_RPW - 1] : max(max(n[0], n[1]), n[2]);   // rows grow with r
+    int nmax = 0;                                                              // rows grow with r; rows >= M have n = 0
+#pragma unroll
+    for (int r = 0; r < TRMV_RPW; ++r) nmax = max(nmax, n[r]);
 
     auto stage = [&](int ch, int buf) {
         const int j0 = ch * TRMV_CHUNK;
