@@ -149,6 +149,43 @@ def test_cholesky_on_general_spd_and_unpadded_ld():
             assert np.linalg.norm(Lg[c] - np.linalg.cholesky(A[c])) / np.linalg.norm(Lg[c]) < 1e-13
 
 
+@pytest.mark.parametrize("N", [341, 455, 699])
+def test_cholesky_recursive_panels_and_trailing_update_against_oracle(N):
+    """M = 1026, 1368, 2100: just past / well past the outer panel width (1024) -> trailing update + second panel, ragged
+    recursion halves (M not a multiple of 64), general SPD input; expected factor from the oracle's row-by-row Cholesky."""
+    M = 3 * (N + 1)
+    rng = np.random.default_rng(N)
+    G = rng.standard_normal((M, M)) / np.sqrt(M)
+    A = G @ G.T + 0.5 * np.eye(M)
+    bd = _bd(N, 1)
+    buf = np.zeros((1, M, bd.ld)); buf[0, :, :M] = A
+    DL = _dev(buf)
+    bd.cholesky(DL)
+    Lg = np.tril(_host(DL)[0, :, :M])
+    Lo, info = O.cholesky(A)
+    assert info == 0
+    assert np.linalg.norm(Lg - Lo) / np.linalg.norm(Lo) <= 1e-12
+    assert np.linalg.norm(Lg @ Lg.T - A) / np.linalg.norm(A) < 1e-12
+
+
+@pytest.mark.parametrize("row", [5, 40, 70, 100, 190])
+def test_cholesky_failing_pivot_row_in_every_part_of_a_block(row):
+    """a non-positive pivot in the first / second half of the first 64-block, in the second block, further down:
+    info must be the oracle's 1-based failing row (reading A10)."""
+    N = 66                                                         # M = 201
+    M = 3 * (N + 1)
+    rng = np.random.default_rng(row)
+    G = rng.standard_normal((M, M)) / np.sqrt(M)
+    A = G @ G.T + 0.5 * np.eye(M)
+    A[row, row] = -1.0                                             # leading minor of order row + 1 is not positive definite
+    bd = _bd(N, 1)
+    buf = np.zeros((1, M, bd.ld)); buf[0, :, :M] = A
+    info = torch.zeros(1, dtype=torch.int32, device="cuda")
+    bd.cholesky(_dev(buf), info)
+    want = O.cholesky(A)[1]
+    assert want == row + 1 and int(_host(info)[0]) == want
+
+
 def test_cholesky_reports_non_positive_pivot():
     """reading A10: bead 2 sits on bead 0 -> D singular at row 7 (exact zero pivot); other chains unaffected."""
     N = 20
