@@ -204,7 +204,7 @@ def test_cholesky_reports_non_positive_pivot():
 
 
 # ------------------------------------------------------------------------------------------ a5
-@pytest.mark.parametrize("N,C", SIZES)
+@pytest.mark.parametrize("N,C", SIZES + [(345, 1), (400, 2)])     # M = 1038, 1203: the shared-memory-staged kernel
 def test_brownian_matches_oracle(N, C):
     r = W.random_chains(C, N, seed=300 + N)
     dt = 1e-4
