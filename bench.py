@@ -241,7 +241,9 @@ def main():
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
             "config": {"workload": w.name, "n_chains_per_gpu": C, "n_rods": w.n_rods, "M": w.M, "dt": w.dt, "hstar": w.hstar,
-                       "flow": w.flow, "Wi": w.Wi, "l2": "inputs larger than L2 (D/L storage %.0f MB per step)" % (bd.workspace_bytes() / 1e6),
+                       "flow": w.flow, "Wi": w.Wi, "l2": ("working set larger than L2 (fragment-major L scratch of the resident CTAs, %.0f MB per step)" %
+                              (min(C, 2 * 148) * ((w.M + 7) // 8 * 8) ** 2 * 8 / 1e6)) if stage["fused"] > 0.0 else
+                             ("inputs larger than L2 (D/L storage %.0f MB per step)" % (bd.workspace_bytes() / 1e6)),
                        "failed_chains": failed},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
             "stage_ms_per_step": stages,
