@@ -90,7 +90,6 @@ __global__ void __launch_bounds__(TRMV_WARPS * 32) k_trmv_staged(int M, const do
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nblk = (M + TRMV_BLK - 1) / TRMV_BLK;
     const int blk = nblk - 1 - blockIdx.x;                                      // longest rows are scheduled first
-    const bool idle = false;
     const int row0 = blk * TRMV_BLK + warp * TRMV_RPW;
     const double* Lc = L_all + (size_t)c * stride;
     const double* dW = dW_all + (size_t)c * M;
@@ -102,7 +101,7 @@ __global__ void __launch_bounds__(TRMV_WARPS * 32) k_trmv_staged(int M, const do
 #pragma unroll
     for (int r = 0; r < TRMV_RPW; ++r) {
         const int row = row0 + r;
-        n[r] = (idle || row >= M) ? 0 : row + 1;
+        n[r] = (row >= M) ? 0 : row + 1;
         Lr[r] = Lc + (size_t)min(row, M - 1) * ld;
         acc[r] = 0.0;
     }

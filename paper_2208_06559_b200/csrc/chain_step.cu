@@ -67,19 +67,8 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
                  : "+d"(c0), "+d"(c1)
                  : "d"(a), "d"(b));
 }
-__device__ __forceinline__ void group_barrier(int id, int nthreads)
-{
-    asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(nthreads) : "memory");
-}
-// ---- shared-window (32-bit address) accessors: no generic-address arithmetic in the latency-critical loops
+// shared-window (32-bit) address of a shared-memory object, for the mbarrier / TMA instructions
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ double lds_f64(uint32_t a)
-{
-    double v;
-    asm volatile("ld.shared.f64 %0, [%1];\n" : "=d"(v) : "r"(a));
-    return v;
-}
-__device__ __forceinline__ void sts_f64(uint32_t a, double v) { asm volatile("st.shared.f64 [%0], %1;\n" ::"r"(a), "d"(v) : "memory"); }
 // ---- mbarrier + TMA bulk copy (global -> shared) ------------------------------------------------------
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 {

@@ -44,8 +44,8 @@ __device__ __forceinline__ void gemm32(const double* __restrict__ X, const doubl
 }
 
 // rows / columns o .. o+31 of the working copy: warp 0 factors (L back into S, 1 / L_kk into s_rinv), warp 1 forms the
-// inverse of that 32 x 32 factor in Wm, 4 pivots behind (named barriers 1..8).  Must be inlined at both call sites:
-// out of line, the per-lane row arrays land in local memory (measured: 29 k instead of 7 k cycles).
+// inverse of that 32 x 32 factor in Wm, 4 pivots behind (named barriers 1..8).  Called from ONE place (a loop over the two
+// halves): the fully unrolled pivot loops are ~1700 straight-line instructions, and a second inlined copy ran 4x slower.
 __device__ __forceinline__ void factor_half(double* __restrict__ S, double* __restrict__ Wm, double* __restrict__ sCol,
                                             double* __restrict__ sRinv, const int o, const int lane, const int warp, const int j0,
                                             int* sFail)
