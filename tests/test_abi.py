@@ -67,3 +67,17 @@ def test_product_does_not_import_the_oracle():
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert "include/bd.h" not in src.replace("(include/bd.h,", "") or True
             assert "import paper_2208" not in src and "from paper_2208" not in src, f
+
+
+def test_user_scripts_import_and_fail_loudly_without_a_gpu():
+    """nsweep / run_config / relaxation are thin drivers of the binding: importable on a CPU box, and they raise
+    (no fallback) as soon as they need a context."""
+    import importlib
+    import torch
+    for name in ("nsweep", "run_config", "relaxation"):
+        mod = importlib.import_module(f"paper_2208_06559_b200.{name}")
+        assert hasattr(mod, "main")
+    if not torch.cuda.is_available():
+        from paper_2208_06559_b200 import relaxation
+        with pytest.raises(RuntimeError):
+            relaxation.measure(5, 2, 0.25, 1e-3, 0.1, 2)
