@@ -28,13 +28,18 @@ OBS_NAMES = ("R2", "Rx2", "Ry2", "Rz2", "Rg2", "Sxx", "Syy", "Szz", "Sxy", "Sxz"
 
 def build(force: bool = False) -> str:
     """Compile the oracle (gcc, no FMA contraction).  Building the checker is not using it."""
-    stale = (not os.path.exists(_LIB)) or any(
-        os.path.getmtime(s) > os.path.getmtime(_LIB) for s in (_SRC, _HDR))
+    # BD_ORACLE_SANITIZE=1: a second build with AddressSanitizer + UBSan for checking the checker itself
+    # (run the CPU tests with LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0).
+    san = bool(os.environ.get("BD_ORACLE_SANITIZE"))
+    out = _LIB.replace(".so", "_san.so") if san else _LIB
+    stale = (not os.path.exists(out)) or any(
+        os.path.getmtime(s) > os.path.getmtime(out) for s in (_SRC, _HDR))
     if force or stale:
-        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-std=c99", "-shared", "-fPIC",
-               "-o", _LIB, _SRC, "-lm"]
+        extra = ["-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"] if san else []
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-std=c99", "-shared", "-fPIC", *extra,
+               "-o", out, _SRC, "-lm"]
         subprocess.run(cmd, check=True, cwd=_HERE)
-    return _LIB
+    return out
 
 
 class _Params(C.Structure):
