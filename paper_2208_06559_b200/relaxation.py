@@ -44,11 +44,24 @@ def measure(n_rods: int, n_chains: int, hstar: float, dt: float, window: float, 
     assert bd.last_info() == (0, -1)
     per = per.cpu().numpy()
     t, acf = np.array(t), np.array(acf)
-    lo = int(0.3 * len(t))                                   # last 70 % of the recorded window
-    ok = acf[lo:] > 0.0
-    slope, _ = np.polyfit(t[lo:][ok], np.log(acf[lo:][ok]), 1)
-    return {"N": n_rods, "hstar": hstar, "lambda": -1.0 / slope, "lambda_rouse": lam_r, "Ree": math.sqrt(per[:, 0].mean()),
-            "Rg": math.sqrt(per[:, 4].mean()), "steps": step, "acf_end": float(acf[-1])}
+    lam, t_cut = fit_tail(t, acf, n_chains)
+    return {"N": n_rods, "hstar": hstar, "lambda": lam, "lambda_rouse": lam_r, "Ree": math.sqrt(per[:, 0].mean()),
+            "Rg": math.sqrt(per[:, 4].mean()), "steps": step, "acf_end": float(acf[-1]), "t_cut": t_cut}
+
+
+def fit_tail(t, acf, n_chains):
+    """lambda from "the last 70 % of the auto-correlation function", where the function ends at t_cut, the
+    first time it drops below its own noise floor max(0.05, 3 / sqrt(chains)) (the standard error of C(t) over the
+    ensemble is ~ 1 / sqrt(chains)); beyond that ln C is noise and a fit over it returns the window, not lambda (the
+    first version fitted the whole recorded window: with HI the function is gone after a tenth of a Rouse time)."""
+    floor = max(0.05, 3.0 / math.sqrt(n_chains))
+    below = np.nonzero(acf < floor)[0]
+    hi = int(below[0]) if len(below) else len(t)
+    lo = int(0.3 * hi)
+    if hi - lo < 3:
+        return float("nan"), float(t[min(hi, len(t) - 1)])
+    slope, _ = np.polyfit(t[lo:hi], np.log(acf[lo:hi]), 1)
+    return -1.0 / slope, float(t[hi - 1])
 
 
 def main():
@@ -57,17 +70,18 @@ def main():
     ap.add_argument("--chains", type=int, default=1024)
     ap.add_argument("--hstar", type=float, nargs="+", default=[0.5, 0.0])
     ap.add_argument("--dt", type=float, default=1e-3)
-    ap.add_argument("--window", type=float, default=2.0, help="length of the run in Rouse relaxation times")
+    ap.add_argument("--window", type=float, default=2.0, help="length of the run in Rouse relaxation times (h* = 0)")
+    ap.add_argument("--window-hi", type=float, default=0.5, help="the same for h* > 0 (relaxation with HI is several times faster)")
     ap.add_argument("--samples", type=int, default=200)
     args = ap.parse_args()
-    print("| h* | N rods | steps | lambda (fit) | Rouse stand-in | R_ee | R_g | C(t_end) |")
-    print("|---|---|---|---|---|---|---|---|")
+    print("| h* | N rods | steps | lambda (fit) | fitted up to t = | Rouse stand-in | R_ee | R_g | C(t_end) |")
+    print("|---|---|---|---|---|---|---|---|---|")
     rows = []
     for h in args.hstar:
         for n in args.rods:
-            row = measure(n, args.chains, h, args.dt, args.window, args.samples)
+            row = measure(n, args.chains, h, args.dt, args.window if h == 0.0 else args.window_hi, args.samples)
             rows.append(row)
-            print(f"| {h} | {n} | {row['steps']} | {row['lambda']:.4g} | {row['lambda_rouse']:.4g} | {row['Ree']:.4g} | {row['Rg']:.4g} | "
+            print(f"| {h} | {n} | {row['steps']} | {row['lambda']:.4g} | {row['t_cut']:.4g} | {row['lambda_rouse']:.4g} | {row['Ree']:.4g} | {row['Rg']:.4g} | "
                   f"{row['acf_end']:.3f} |", flush=True)
     for h in args.hstar:
         sel = [r for r in rows if r["hstar"] == h]

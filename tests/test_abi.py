@@ -70,14 +70,31 @@ def test_product_does_not_import_the_oracle():
 
 
 def test_user_scripts_import_and_fail_loudly_without_a_gpu():
-    """nsweep / run_config / relaxation are thin drivers of the binding: importable on a CPU box, and they raise
+    """nsweep / run_config / relaxation / variant_sweep are thin drivers of the binding: importable on a CPU box, and they raise
     (no fallback) as soon as they need a context."""
     import importlib
     import torch
-    for name in ("nsweep", "run_config", "relaxation"):
+    for name in ("nsweep", "run_config", "relaxation", "variant_sweep"):
         mod = importlib.import_module(f"paper_2208_06559_b200.{name}")
         assert hasattr(mod, "main")
     if not torch.cuda.is_available():
         from paper_2208_06559_b200 import relaxation
         with pytest.raises(RuntimeError):
             relaxation.measure(5, 2, 0.25, 1e-3, 0.1, 2)
+
+
+def test_relaxation_fit_stops_at_the_noise_floor():
+    """host logic of relaxation.py: lambda from the last 70 % of the RESOLVED part of C(t).  A synthetic
+    exp(-t / lambda) with ensemble noise 1 / sqrt(chains), recorded far beyond its decay, must return lambda -- a fit over
+    the whole window returns the window length instead (what the first version did for the runs with HI)."""
+    import math
+    import numpy as np
+    from paper_2208_06559_b200.relaxation import fit_tail
+    rng = np.random.default_rng(5)
+    t = np.linspace(0.0, 440.0, 201)
+    for lam in (25.0, 90.0, 280.0):
+        acf = np.exp(-t / lam) + rng.normal(0.0, 1.0 / math.sqrt(2048), t.size)
+        acf[0] = 1.0
+        fit, t_cut = fit_tail(t, acf, 2048)
+        assert abs(fit - lam) <= 0.08 * lam
+        assert t_cut <= min(440.0, 3.5 * lam)

@@ -305,6 +305,27 @@ def test_fused_and_staged_paths_agree():
     assert np.abs(outs[0] - outs[1]).max() / np.abs(outs[0]).max() <= 1e-11
 
 
+@pytest.mark.parametrize("path,name", PATHS)
+def test_negligible_hstar_follows_the_free_draining_run(path, name):
+    """PAPER.md:262 / Fig. 6 (:419): with h* = 1e-5 the run with HI must agree with the run without HI (same start,
+    same noise).  D = I + O(h*), so L = I + O(h*): after 200 steps of the paper's variant (uniform noise, dt = 1e-3,
+    K* = 1e3, extension) the two differ by O(h* x displacement), and each tracks the oracle at its own h*."""
+    N, C, dt, steps = 100, 4, 1e-3, 200
+    kappa = np.diag([0.01, -0.005, -0.005])
+    r0 = W.random_chains(C, N, seed=61, rod_jitter=0.0)
+    out = {}
+    for h in (1e-5, 0.0):
+        bd = _bd(N, C, dt, hstar=h, kappa=kappa, seed=3, noise_kind=1)
+        bd.set_path(path)
+        out[h] = _host(bd.step(_dev(r0), 0, steps))
+        assert bd.last_info() == (0, -1)
+        assert _step_parity(N, 2, dt, h, kappa, steps=1, noise_kind=1, seed=3, jitter=0.0, rseed=61, path=path)[0] <= 1e-10
+    moved = np.abs(out[0.0] - r0).max()
+    diff = np.abs(out[1e-5] - out[0.0]).max()
+    assert moved > 0.5                                           # the chains did move (200 steps of sqrt(2 dt) kicks)
+    assert 0.0 < diff <= 1e-3 * moved                            # HI is ON (diff > 0) but negligible
+
+
 def test_fused_path_rejected_for_long_chains():
     from paper_2208_06559_b200.binding import BDError
     bd = _bd(200, 1)
