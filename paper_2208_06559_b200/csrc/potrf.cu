@@ -363,10 +363,7 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
     const int n = ctx->M, C = ctx->C;
     // outer panel width, from sweeps on B200 (profiles/r01_summary.md): with the recursive panel below, wide outer
     // panels win (c4: 256 -> 0.641, 1024 -> 0.688, 4096 -> 0.695 of peak; c5: 0.686 / 0.769 / 0.781)
-    int NB = (n >= 4096) ? 4096 : 1024;
-    static const int exp_nb = getenv("BD_EXP_NB") ? atoi(getenv("BD_EXP_NB")) : 0;
-    static const int exp_lb = getenv("BD_EXP_LB") ? atoi(getenv("BD_EXP_LB")) : 0;
-    if (exp_nb > 0) NB = exp_nb;
+    const int NB = (n >= 4096) ? 4096 : 1024;
     // Outer level: right-looking.  A left-looking outer loop (block column J updated by all finished columns in one
     // pass, K = J; kept behind `left`) measured equal at c3 / c4 and slower at c5 (0.78 -> 0.75: the K-deep operand
     // streams of all row blocks no longer share L2).
@@ -376,23 +373,9 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
     // block updated once per preceding block, always K = 64, DMMA pipe ~50 % busy) each column block now sees
     // log2((J1 - J0) / 64) updates with K = 64, 128, 256, ..
     struct Rec {
-        bd_ctx* ctx; double* A; int64_t ld, stride; int32_t* info; int n, C, trsm_smem, lb;
+        bd_ctx* ctx; double* A; int64_t ld, stride; int32_t* info; int n, C, trsm_smem;
         int run(int J0, int J1)
         {
-            if (lb > 0 && J1 - J0 > lb) {
-                // left-looking over lb-column blocks: block j is updated ONCE by all finished columns of this panel (K = j - J0)
-                const int keep = lb;
-                for (int j = J0; j < J1; j += keep) {
-                    const int je = (j + keep < J1) ? j + keep : J1;
-                    int rc;
-                    if (j > J0 && (rc = launch_syrk(ctx, A, ld, stride, j, n, je, J0, j - J0)) != 0) return rc;
-                    lb = 0;
-                    rc = run(j, je);
-                    lb = keep;
-                    if (rc != 0) return rc;
-                }
-                return 0;
-            }
             if (J1 - J0 <= BD_NB_INNER) {
                 const int nloc = J1 - J0;
                 BD_LAUNCH(ctx, k_potf2, dim3(C), dim3(256), potf2::SMEM_BYTES, A, ld, stride, J0, nloc, info, ctx->Winv);
@@ -408,7 +391,7 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
             if ((rc = launch_syrk(ctx, A, ld, stride, mid, n, J1, J0, half)) != 0) return rc;
             return run(mid, J1);
         }
-    } rec{ctx, A, ld, stride, info, n, C, trsm_smem, exp_lb};
+    } rec{ctx, A, ld, stride, info, n, C, trsm_smem};
     for (int J = 0; J < n; J += NB) {
         const int Jend = (J + NB < n) ? J + NB : n;
         if (left && J > 0) {
