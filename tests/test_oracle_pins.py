@@ -483,6 +483,55 @@ def test_observables_closed_forms():
     assert o["Sxx"] == pytest.approx(o["Syy"]) and o["Sxz"] == 0
 
 
+def test_observables_generic_position_every_component_distinct():
+    """Eqs. 25-28 written out by hand for a 2-rod chain in GENERAL position, so that every one of the
+    13 outputs is a distinct non-zero number (a y<->z swap, or a swapped pair of stress indices, fails here):
+        r_0 = (0,0,0), Q_0 = (0.3, 0.4, 1.2) (|Q_0| = 1.3), Q_1 = (-0.6, 0.2, 0.3) (|Q_1| = 0.7), b = 1, K = 100.
+    End to end R = Q_0 + Q_1 = (-0.3, 0.6, 1.5); centre of mass (0, 1/3, 0.9);
+    T_k = K (|Q_k| - b)/|Q_k| Q_k: c_0 = 100 * 0.3/1.3 = 300/13, c_1 = 100 * (-0.3)/0.7 = -300/7 (Eq. 3);
+    S = c_0 Q_0 Q_0^T + c_1 Q_1 Q_1^T (Eq. 28 without N delta)."""
+    from fractions import Fraction as Fr
+    r = np.array([[[0, 0, 0], [0.3, 0.4, 1.2], [-0.3, 0.6, 1.5]]], dtype=float)
+    o = dict(zip(O.OBS_NAMES, O.observables(_params(2, K=100.0), r)[0][0]))
+    c0, c1 = Fr(300, 13), Fr(-300, 7)
+    want = {
+        "Rx2": Fr(9, 100), "Ry2": Fr(36, 100), "Rz2": Fr(225, 100), "R2": Fr(270, 100),
+        # sum_i |r_i - cm|^2 = (0 + 1/9 + 81/100) + (9/100 + 1/225 + 9/100) + (9/100 + 16/225 + 36/100) = 122/75
+        "Rg2": Fr(122, 225),
+        "Sxx": c0 * Fr(9, 100) + c1 * Fr(36, 100),
+        "Syy": c0 * Fr(16, 100) + c1 * Fr(4, 100),
+        "Szz": c0 * Fr(144, 100) + c1 * Fr(9, 100),
+        "Sxy": c0 * Fr(12, 100) + c1 * Fr(-12, 100),
+        "Sxz": c0 * Fr(36, 100) + c1 * Fr(-18, 100),
+        "Syz": c0 * Fr(48, 100) + c1 * Fr(6, 100),
+        "rod_dev_ms": Fr(9, 100), "rod_dev_max": Fr(3, 10),
+    }
+    vals = [float(v) for k, v in want.items() if not k.startswith("rod_dev")]
+    assert len({round(abs(v), 9) for v in vals}) == len(vals)          # the 11 R / Rg / S entries are pairwise distinct
+    for k, v in want.items():
+        assert o[k] == pytest.approx(float(v), rel=1e-12), k
+
+
+def test_initial_walk_follows_the_purpose_one_counter_layout():
+    """Reading A13 / DESIGN.md section 3: link k of chain c comes from the KAT-pinned Philox block function with counter
+    (k, c, step 0, purpose 1 << 28), key = (init_seed lo, hi): z = 2 u1 - 1, phi = 2 pi u2,
+    Q_k = b (sqrt(1 - z^2) cos phi, sqrt(1 - z^2) sin phi, z).  Recomputed here, link by link."""
+    N, b, seed, chain = 9, 1.7, 0xABCDEF01_23456789, 41
+    r = O.init_random_walk(N, b, seed, [chain])[0]
+    assert np.allclose(r.mean(0), 0.0, atol=1e-14)
+    Q = np.diff(r, axis=0)
+    for k in range(N):
+        w = O.philox4x32_10([k, chain, 0, 1 << 28], [seed & 0xFFFFFFFF, seed >> 32])
+        x1, x2 = (w[1] << 32) | w[0], (w[3] << 32) | w[2]
+        u1, u2 = (2 * (x1 >> 12) + 1) / 2.0 ** 53, (2 * (x2 >> 12) + 1) / 2.0 ** 53
+        z, phi = 2.0 * u1 - 1.0, 6.283185307179586 * u2
+        s = math.sqrt(1.0 - z * z)
+        assert Q[k] == pytest.approx([b * s * math.cos(phi), b * s * math.sin(phi), b * z], rel=1e-13, abs=1e-14)
+    # purpose 0 (the noise stream) with the same key / chain / pair gives different words
+    assert O.philox4x32_10([0, chain, 0, 0], [seed & 0xFFFFFFFF, seed >> 32]) != \
+        O.philox4x32_10([0, chain, 0, 1 << 28], [seed & 0xFFFFFFFF, seed >> 32])
+
+
 def test_failure_leaves_state_unchanged():
     """A10: coincident beads with h* = a make D singular -> reported, state untouched."""
     r = np.array([[0, 0, 0], [1.0, 0, 0], [0, 0, 0]], dtype=float)     # bead 2 on top of bead 0
