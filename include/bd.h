@@ -148,7 +148,13 @@ int bd_stage_ms(bd_ctx *ctx, double ms_host[BD_NSTAGES], int64_t *steps_host);
 /* Number of kernel launches issued through this context so far (for bench.py's gpu_launches).   */
 int64_t bd_launch_count(const bd_ctx *ctx);
 
+/* Text for a return code.  For BD_ERR_CUDA raised by bd_create (no context yet) the CUDA error text of the calling
+ * thread's last failed bd_create; for BD_ERR_CUDA from any other call use bd_last_error.                            */
 const char *bd_strerror(int code);
+
+/* Text of the last CUDA error recorded in this context (errors are per context; the library keeps no
+ * process-wide state).                                                                                */
+const char *bd_last_error(const bd_ctx *ctx);
 
 #ifdef __cplusplus
 }

@@ -29,7 +29,7 @@ class bd_params(C.Structure):
 EXPORTS = ("bd_create", "bd_destroy", "bd_workspace_bytes", "bd_set_workspace", "bd_set_flow",
            "bd_init_random_walk", "bd_assemble_hi", "bd_cholesky", "bd_brownian", "bd_noise", "bd_drift",
            "bd_update", "bd_set_path", "bd_step", "bd_observables", "bd_last_info", "bd_step_host", "bd_profile",
-           "bd_stage_ms", "bd_launch_count", "bd_strerror")
+           "bd_stage_ms", "bd_launch_count", "bd_strerror", "bd_last_error")
 
 _lib = None
 
@@ -68,8 +68,10 @@ def load_library(path: str | None = None) -> C.CDLL:
     lib.bd_launch_count.restype = i64
     lib.bd_strerror.argtypes = [C.c_int]
     lib.bd_strerror.restype = C.c_char_p
+    lib.bd_last_error.argtypes = [vp]
+    lib.bd_last_error.restype = C.c_char_p
     for name in EXPORTS:
-        if name not in ("bd_workspace_bytes", "bd_launch_count", "bd_strerror"):
+        if name not in ("bd_workspace_bytes", "bd_launch_count", "bd_strerror", "bd_last_error"):
             getattr(lib, name).restype = C.c_int
     if path is None:
         _lib = lib
@@ -118,7 +120,10 @@ class BD:
     # ------------------------------------------------------------------ helpers
     def _check(self, fn: str, rc: int):
         if rc != 0:
-            raise BDError(fn, rc, self.lib.bd_strerror(rc).decode())
+            text = self.lib.bd_strerror(rc).decode()
+            if rc == ERR_CUDA and getattr(self, "_ctx", None) is not None and self._ctx.value:
+                text = self.lib.bd_last_error(self._ctx).decode()
+            raise BDError(fn, rc, text)
 
     def close(self):
         if getattr(self, "_ctx", None) is not None and self._ctx.value:

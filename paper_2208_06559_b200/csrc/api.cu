@@ -19,7 +19,9 @@ bool layout_ok(const bd_ctx* ctx, const void* p, int64_t ld, int64_t stride)
 
 }  // namespace
 
-cudaError_t bd_g_last_cuda = cudaSuccess;
+// bd_create can fail before a context exists: its CUDA error is kept per calling thread for bd_strerror.  Every other
+// CUDA error lives in the context (bd_last_error).
+static thread_local cudaError_t tl_create_cuda = cudaSuccess;
 
 extern "C" {
 
@@ -29,7 +31,7 @@ int bd_create(const bd_params* params, void* cuda_stream, bd_ctx** out)
     if (out == nullptr) return -3;
     *out = nullptr;
     bd_params p = *params;
-    if (p.n_rods < 1 || p.n_chains < 1 || p.n_chains > 65535) return -1;
+    if (p.n_rods < 1 || p.n_chains < 1) return -1;
     if (!(p.b > 0.0) || !(p.hstar >= 0.0) || !(p.dt > 0.0) || !std::isfinite(p.b) || !std::isfinite(p.hstar) || !std::isfinite(p.dt))
         return -1;
     if (!(p.a > 0.0)) p.a = p.hstar * p.b;                 // reading A3: a = h* b
@@ -43,7 +45,7 @@ int bd_create(const bd_params* params, void* cuda_stream, bd_ctx** out)
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
-        bd_g_last_cuda = cudaGetLastError();
+        tl_create_cuda = cudaGetLastError();
         return BD_ERR_CUDA;                               // no host fallback, by design
     }
     bd_ctx* ctx = new (std::nothrow) bd_ctx();
@@ -60,7 +62,7 @@ int bd_create(const bd_params* params, void* cuda_stream, bd_ctx** out)
     int dev = 0;
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
-        bd_g_last_cuda = cudaGetLastError();
+        tl_create_cuda = cudaGetLastError();
         delete ctx;
         return BD_ERR_CUDA;
     }
@@ -75,6 +77,7 @@ int bd_create(const bd_params* params, void* cuda_stream, bd_ctx** out)
         {(void**)&ctx->tmp, sizeof(double) * CM},
         {(void**)&ctx->r_own, sizeof(double) * CM},
         {(void**)&ctx->info, sizeof(int32_t) * (size_t)ctx->C},
+        {(void**)&ctx->info_step, sizeof(int32_t) * (size_t)ctx->C},
         {(void**)&ctx->fail, sizeof(int32_t) * 2},
         {(void**)&ctx->obs, sizeof(double) * ((size_t)ctx->C + 2) * BD_NOBS},
         {(void**)&ctx->Winv, sizeof(double) * (size_t)ctx->C * BD_NB_INNER * BD_NB_INNER},
@@ -82,7 +85,7 @@ int bd_create(const bd_params* params, void* cuda_stream, bd_ctx** out)
     for (auto& al : allocs) {
         cudaError_t e = cudaMalloc(al.p, al.bytes);
         if (e != cudaSuccess) {
-            bd_g_last_cuda = e;
+            tl_create_cuda = e;
             bd_destroy(ctx);
             return BD_ERR_CUDA;
         }
@@ -90,7 +93,7 @@ int bd_create(const bd_params* params, void* cuda_stream, bd_ctx** out)
     cudaError_t e = cudaMemsetAsync(ctx->info, 0, sizeof(int32_t) * (size_t)ctx->C, ctx->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
     if (e != cudaSuccess) {
-        bd_g_last_cuda = e;
+        tl_create_cuda = e;
         bd_destroy(ctx);
         return BD_ERR_CUDA;
     }
@@ -102,7 +105,7 @@ int bd_destroy(bd_ctx* ctx)
 {
     if (ctx == nullptr) return -1;
     cudaStreamSynchronize(ctx->stream);
-    void* ptrs[] = {ctx->T, ctx->F, ctx->v, ctx->y, ctx->dW, ctx->tmp, ctx->r_own, ctx->info, ctx->fail, ctx->obs, ctx->Winv};
+    void* ptrs[] = {ctx->T, ctx->F, ctx->v, ctx->y, ctx->dW, ctx->tmp, ctx->r_own, ctx->info, ctx->info_step, ctx->fail, ctx->obs, ctx->Winv};
     for (void* q : ptrs)
         if (q != nullptr) cudaFree(q);
     if (ctx->ev != nullptr) {
@@ -205,7 +208,7 @@ int bd_update(bd_ctx* ctx, const double* r_dev, const double* v_dev, const doubl
     if (v_dev == nullptr) return -3;
     if (y_dev == nullptr) return -4;
     if (r_out_dev == nullptr) return -5;
-    return bdk_update(ctx, r_dev, v_dev, y_dev, nullptr, ctx->info, r_out_dev);
+    return bdk_update(ctx, r_dev, v_dev, y_dev, nullptr, ctx->info, r_out_dev);   // a non-finite update is recorded in the sticky info
 }
 
 int bd_step(bd_ctx* ctx, double* r_dev, uint64_t first_step, int32_t n_steps)
@@ -237,18 +240,21 @@ int bd_step(bd_ctx* ctx, double* r_dev, uint64_t first_step, int32_t n_steps)
             ev = ctx->ev + (size_t)(ctx->ev_steps++) * (BD_NSTAGES + 1);
         }
 #define BD_MARK(i) do { if (ev != nullptr) BD_CUDA(ctx, cudaEventRecord(ev[i], ctx->stream)); } while (0)
+        // reading A10: a failed chain keeps its positions FOR THAT STEP and is tried again in the next one (as the fused
+        // kernel and the oracle do): failures of this step go to info_step, the first failure of a chain stays in info
+        BD_CUDA(ctx, cudaMemsetAsync(ctx->info_step, 0, sizeof(int32_t) * (size_t)ctx->C, ctx->stream));
         BD_MARK(0);
         if ((rc = bdk_drift(ctx, r_dev, nullptr, ctx->F, ctx->v)) != 0) return rc;                       // a1, a4
         BD_MARK(1);
         if ((rc = bdk_assemble(ctx, r_dev, ctx->ws, ctx->ws_ld, ctx->ws_stride, 0)) != 0) return rc;     // a2
         BD_MARK(2);
-        if ((rc = bdk_potrf(ctx, ctx->ws, ctx->ws_ld, ctx->ws_stride, ctx->info)) != 0) return rc;       // a3
+        if ((rc = bdk_potrf(ctx, ctx->ws, ctx->ws_ld, ctx->ws_stride, ctx->info_step)) != 0) return rc;  // a3
         BD_MARK(3);
         if ((rc = bdk_noise(ctx, first_step + (uint64_t)s, ctx->dW)) != 0) return rc;                    // a0
         BD_MARK(4);
         if ((rc = bdk_trmv(ctx, ctx->ws, ctx->ws_ld, ctx->ws_stride, ctx->dW, ctx->y)) != 0) return rc;  // a5
         BD_MARK(5);
-        if ((rc = bdk_update(ctx, r_dev, ctx->v, ctx->y, ctx->info, ctx->info, r_dev)) != 0) return rc;  // a6-a8
+        if ((rc = bdk_update(ctx, r_dev, ctx->v, ctx->y, ctx->info_step, ctx->info, r_dev)) != 0) return rc;  // a6-a8
         BD_MARK(6);
 #undef BD_MARK
     }
@@ -348,11 +354,17 @@ int bd_stage_ms(bd_ctx* ctx, double ms_host[BD_NSTAGES], int64_t* steps_host)
 
 int64_t bd_launch_count(const bd_ctx* ctx) { return (ctx == nullptr) ? 0 : ctx->launches; }
 
+const char* bd_last_error(const bd_ctx* ctx)
+{
+    if (ctx == nullptr) return "no context";
+    return (ctx->last_cuda == cudaSuccess) ? "no CUDA error recorded" : cudaGetErrorString(ctx->last_cuda);
+}
+
 const char* bd_strerror(int code)
 {
     switch (code) {
         case 0: return "success";
-        case BD_ERR_CUDA: return (bd_g_last_cuda != cudaSuccess) ? cudaGetErrorString(bd_g_last_cuda) : "CUDA runtime error (see cudaGetLastError)";
+        case BD_ERR_CUDA: return (tl_create_cuda != cudaSuccess) ? cudaGetErrorString(tl_create_cuda) : "CUDA runtime error (bd_last_error(ctx) gives the text)";
         case BD_ERR_WORKSPACE: return "bd_step needs a workspace: call bd_set_workspace first";
         case BD_ERR_ALLOC: return "host allocation failed";
         default: break;

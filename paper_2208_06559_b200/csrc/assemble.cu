@@ -23,7 +23,7 @@ __global__ void __launch_bounds__(TI * TJ) k_assemble(int Nb, double hstar, doub
     const int i0 = blockIdx.y * TI, j0 = blockIdx.x * TJ;
     if (j0 > i0 + TI - 1) return;                       // tile entirely above the diagonal
     __shared__ __align__(16) double s_tile[TROWS][TLD];
-    const int c = blockIdx.z;
+    const int c = blockIdx.z;                           // the host launches at most 65535 chains at a time
     const int M = 3 * Nb;
     const double* r = r_all + (size_t)c * M;
     double* D = D_all + (size_t)c * stride;
@@ -76,8 +76,13 @@ __global__ void __launch_bounds__(TI * TJ) k_assemble(int Nb, double hstar, doub
 
 int bdk_assemble(bd_ctx* ctx, const double* r, double* D, int64_t ld, int64_t stride, int full)
 {
-    dim3 grid((ctx->Nb + TJ - 1) / TJ, (ctx->Nb + TI - 1) / TI, ctx->C);
-    BD_LAUNCH(ctx, k_assemble, grid, dim3(TI * TJ), 0, ctx->Nb, ctx->p.hstar, ctx->p.a / ctx->p.b, ctx->p.b / ctx->p.a, 1.0 / ctx->p.b, r, D, ld,
-              stride, full);
+    // grid.z carries the chain and is limited to 65535: larger ensembles go in slices (a block index decoded with
+    // integer divisions instead cost 10 % of this short, store-bound kernel)
+    for (int c0 = 0; c0 < ctx->C; c0 += 65535) {
+        const int nc = (ctx->C - c0 < 65535) ? ctx->C - c0 : 65535;
+        dim3 grid((ctx->Nb + TJ - 1) / TJ, (ctx->Nb + TI - 1) / TI, nc);
+        BD_LAUNCH(ctx, k_assemble, grid, dim3(TI * TJ), 0, ctx->Nb, ctx->p.hstar, ctx->p.a / ctx->p.b, ctx->p.b / ctx->p.a, 1.0 / ctx->p.b,
+                  r + (size_t)c0 * ctx->M, D + (size_t)c0 * stride, ld, stride, full);
+    }
     return 0;
 }

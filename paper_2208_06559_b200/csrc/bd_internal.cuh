@@ -20,7 +20,8 @@ struct bd_ctx {
     double* y;              // [C][M]
     double* dW;             // [C][M]
     double* Winv;           // [C][NB_INNER*NB_INNER] inverse of the current diagonal block
-    int32_t* info;          // [C]
+    int32_t* info;          // [C] sticky: first failure of every chain since the last reset (bd_last_info)
+    int32_t* info_step;     // [C] failures of the current time step only (staged bd_step; reading A10: a chain is retried every step)
     int32_t* fail;          // [2]: count, first chain
     double* obs;            // [C][BD_NOBS] + [2][BD_NOBS]
     double* tmp;            // [C][M] unshifted positions inside the update / init kernels
@@ -36,8 +37,6 @@ struct bd_ctx {
     bool attr_potrf, attr_chain;   // cudaFuncSetAttribute done for this context's device (no process-wide statics)
 };
 
-extern cudaError_t bd_g_last_cuda;   // last CUDA error seen by any libbd call (for bd_strerror)
-
 #define BD_NB_INNER 64      // width of the diagonal block factored by potf2 (one CTA per chain)
 
 #define BD_CUDA(ctx, call)                                  \
@@ -45,7 +44,6 @@ extern cudaError_t bd_g_last_cuda;   // last CUDA error seen by any libbd call (
         cudaError_t e__ = (call);                           \
         if (e__ != cudaSuccess) {                           \
             (ctx)->last_cuda = e__;                         \
-            bd_g_last_cuda = e__;                           \
             return BD_ERR_CUDA;                             \
         }                                                   \
     } while (0)
@@ -58,7 +56,6 @@ extern cudaError_t bd_g_last_cuda;   // last CUDA error seen by any libbd call (
         cudaError_t e__ = cudaGetLastError();                                   \
         if (e__ != cudaSuccess) {                                               \
             (ctx)->last_cuda = e__;                                             \
-            bd_g_last_cuda = e__;                                               \
             return BD_ERR_CUDA;                                                 \
         }                                                                       \
     } while (0)
@@ -70,8 +67,8 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
 int bdk_noise(bd_ctx* ctx, uint64_t step, double* dW);
 int bdk_trmv(bd_ctx* ctx, const double* L, int64_t ld, int64_t stride, const double* dW, double* y);
 int bdk_drift(bd_ctx* ctx, const double* r, double* T, double* F, double* v);
-int bdk_update(bd_ctx* ctx, const double* r, const double* v, const double* y, const int32_t* info,
-               int32_t* info_out, double* r_out);
+int bdk_update(bd_ctx* ctx, const double* r, const double* v, const double* y, const int32_t* info_step,
+               int32_t* info_sticky, double* r_out);
 int bdk_observables(bd_ctx* ctx, const double* r, double* per_chain, double* ensemble);
 int bdk_count_failures(bd_ctx* ctx, const int32_t* info);
 bool bdk_chain_step_supported(const bd_ctx* ctx);

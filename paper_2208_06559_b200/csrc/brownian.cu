@@ -6,11 +6,11 @@
 namespace {
 
 // one thread per pair p: dW[2p], dW[2p+1]
-__global__ void __launch_bounds__(256) k_noise(int M, uint64_t seed, uint64_t chain0, uint64_t step, int kind,
+__global__ void __launch_bounds__(256) k_noise(int M, int nblk, uint64_t seed, uint64_t chain0, uint64_t step, int kind,
                                                double dt, double* __restrict__ dW_all)
 {
-    const int c = blockIdx.y;
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    const int c = blockIdx.x / nblk;                       // chain and block both on grid.x: no 65535-chain limit
+    const int p = (blockIdx.x - c * nblk) * blockDim.x + threadIdx.x;
     if (2 * p >= M) return;
     double w0, w1;
     brownian_pair(seed, (uint32_t)p, chain0 + (uint64_t)c, step, kind, dt, w0, w1);
@@ -26,14 +26,14 @@ constexpr int kTrmvWarps = 8;
 __global__ void __launch_bounds__(kTrmvWarps * 32) k_trmv(int M, const double* __restrict__ L_all, int64_t ld, int64_t stride,
                                                          const double* __restrict__ dW_all, double* __restrict__ y_all)
 {
-    const int c = blockIdx.y;
+    const int nblk = (M + kTrmvWarps - 1) / kTrmvWarps;
+    const int c = blockIdx.x / nblk, bx = blockIdx.x - c * nblk;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     // pair short rows with long rows: CTA b takes rows b*4..b*4+3 from the top and the mirrored rows
-    const int nblk = gridDim.x;
     const int half = nblk * (kTrmvWarps / 2);
     int row;
-    if (warp < kTrmvWarps / 2) row = blockIdx.x * (kTrmvWarps / 2) + warp;
-    else row = 2 * half - 1 - (blockIdx.x * (kTrmvWarps / 2) + (warp - kTrmvWarps / 2));
+    if (warp < kTrmvWarps / 2) row = bx * (kTrmvWarps / 2) + warp;
+    else row = 2 * half - 1 - (bx * (kTrmvWarps / 2) + (warp - kTrmvWarps / 2));
     if (row >= M) return;
     const double* Lr = L_all + (size_t)c * stride + (size_t)row * ld;
     const double* dW = dW_all + (size_t)c * M;
@@ -72,24 +72,17 @@ __global__ void __launch_bounds__(kTrmvWarps * 32) k_trmv(int M, const double* _
 // HBM copy peak 6553): one row per warp 4945 / 5073 / 4265; this kernel with 4 rows per warp 4500 / 4540 / 4560, with
 // 1 row per warp - / 5524 / 5995, with 2 rows per warp 5186 / 5454 / 6042 (fewer rows per CTA = a finer tail); pairing a
 // long with a short block per CTA: 4037 at c5 (half the CTAs, half the bytes in flight).  Lanes read 16-byte pairs.
-#ifndef TRMV_MIN_M_N
-#define TRMV_MIN_M_N 1024
-#endif
-constexpr int TRMV_STAGED_MIN_M = TRMV_MIN_M_N;   // below: one row per warp, dW through L1
-#ifndef TRMV_RPW_N
-#define TRMV_RPW_N 2
-#define TRMV_CHUNK_N 2048
-#endif
-constexpr int TRMV_WARPS = 8, TRMV_RPW = TRMV_RPW_N, TRMV_BLK = TRMV_WARPS * TRMV_RPW, TRMV_CHUNK = TRMV_CHUNK_N;
+constexpr int TRMV_STAGED_MIN_M = 1024;           // below: one row per warp, dW through L1
+constexpr int TRMV_WARPS = 8, TRMV_RPW = 2, TRMV_BLK = TRMV_WARPS * TRMV_RPW, TRMV_CHUNK = 2048;
 
 __global__ void __launch_bounds__(TRMV_WARPS * 32) k_trmv_staged(int M, const double* __restrict__ L_all, int64_t ld, int64_t stride,
                                                          const double* __restrict__ dW_all, double* __restrict__ y_all)
 {
     __shared__ __align__(16) double s_w[2][TRMV_CHUNK];
-    const int c = blockIdx.y;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nblk = (M + TRMV_BLK - 1) / TRMV_BLK;
-    const int blk = nblk - 1 - blockIdx.x;                                      // longest rows are scheduled first
+    const int c = blockIdx.x / nblk;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int blk = nblk - 1 - (blockIdx.x - c * nblk);                         // longest rows are scheduled first
     const int row0 = blk * TRMV_BLK + warp * TRMV_RPW;
     const double* Lc = L_all + (size_t)c * stride;
     const double* dW = dW_all + (size_t)c * M;
@@ -156,7 +149,8 @@ __global__ void __launch_bounds__(TRMV_WARPS * 32) k_trmv_staged(int M, const do
 int bdk_noise(bd_ctx* ctx, uint64_t step, double* dW)
 {
     const int pairs = (ctx->M + 1) / 2;
-    BD_LAUNCH(ctx, k_noise, dim3((pairs + 255) / 256, ctx->C), dim3(256), 0, ctx->M, ctx->p.seed, ctx->p.chain_id0, step,
+    const int nblk = (pairs + 255) / 256;
+    BD_LAUNCH(ctx, k_noise, dim3((unsigned)((int64_t)nblk * ctx->C)), dim3(256), 0, ctx->M, nblk, ctx->p.seed, ctx->p.chain_id0, step,
               ctx->p.noise_kind, ctx->p.dt, dW);
     return 0;
 }
@@ -165,10 +159,10 @@ int bdk_trmv(bd_ctx* ctx, const double* L, int64_t ld, int64_t stride, const dou
 {
     if (ctx->M > TRMV_STAGED_MIN_M) {
         const int nb = (ctx->M + TRMV_BLK - 1) / TRMV_BLK;
-        BD_LAUNCH(ctx, k_trmv_staged, dim3(nb, ctx->C), dim3(TRMV_WARPS * 32), 0, ctx->M, L, ld, stride, dW, y);
+        BD_LAUNCH(ctx, k_trmv_staged, dim3((unsigned)((int64_t)nb * ctx->C)), dim3(TRMV_WARPS * 32), 0, ctx->M, L, ld, stride, dW, y);
         return 0;
     }
     const int nblk = (ctx->M + kTrmvWarps - 1) / kTrmvWarps;
-    BD_LAUNCH(ctx, k_trmv, dim3(nblk, ctx->C), dim3(kTrmvWarps * 32), 0, ctx->M, L, ld, stride, dW, y);
+    BD_LAUNCH(ctx, k_trmv, dim3((unsigned)((int64_t)nblk * ctx->C)), dim3(kTrmvWarps * 32), 0, ctx->M, L, ld, stride, dW, y);
     return 0;
 }

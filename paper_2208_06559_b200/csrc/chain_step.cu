@@ -19,7 +19,6 @@
 // Finished rows of L are never needed again (left-looking), so the working set in L2 is small and
 // stays resident while the CTA moves on to its next chain.
 // After the last panel the CTA applies the semi-implicit rod update (Eqs. 14, 17, 15, :139-160).
-#include <cstdlib>
 #include <type_traits>
 
 #include "bd_internal.cuh"
@@ -29,24 +28,12 @@
 
 namespace {
 
-// Optional phase timing (compile with -DCS_PROFILE): thread 0 of every CTA accumulates clock64() deltas
-// per phase into dbg[blockIdx.x][8].
-#ifdef CS_PROFILE
-#define CS_TIC(i) do { if (tid == 0) { long long now__ = clock64(); prof[i] += now__ - tprev; tprev = now__; } } while (0)
-#else
-#define CS_TIC(i) do { } while (0)
-#endif
-
 constexpr int CS_THREADS = 256;
 constexpr int CS_WARPS = 8;
 constexpr int CS_MTW = 5;                 // m-tiles per warp  -> M <= 8*8*5 = 320
 constexpr int CS_MAXM = 8 * CS_WARPS * CS_MTW;
-#ifndef CS_KG_N
-#define CS_KG_N 2
-#define CS_STAGES_N 2
-#endif
-constexpr int CS_KG = CS_KG_N;            // k-groups per ring stage: one mbarrier round trip (~90 cycles) per CS_KG k-groups
-constexpr int CS_STAGES = CS_STAGES_N;    // ring stages
+constexpr int CS_KG = 2;                  // k-groups per ring stage: one mbarrier round trip (~90 cycles) per CS_KG k-groups
+constexpr int CS_STAGES = 2;              // ring stages
 
 struct ChainStepParams {
     int N, C;
@@ -58,7 +45,6 @@ struct ChainStepParams {
     double* scratch;      // per-CTA L storage, fragment-major, MP*MP doubles each
     int64_t scratch_stride;
     int32_t* info;        // [C]
-    long long* dbg;       // CS_PROFILE only
 };
 
 __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
@@ -136,10 +122,6 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
     auto TIDX = [&](int r, int c) { return (c >> 2) * MT4 + r * 4 + (c & 3); };
 
     double* Lg = P.scratch + (size_t)blockIdx.x * P.scratch_stride;
-#ifdef CS_PROFILE
-    long long prof[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    long long tprev = clock64();
-#endif
     const uint32_t bar_full = smem_u32(&sBar[0]), bar_empty = smem_u32(&sBar[CS_STAGES]);
     const uint32_t ring_u32 = smem_u32(ring);
     if (tid == 0) {
@@ -182,7 +164,6 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
             for (int i = tid; i < MP; i += CS_THREADS) sY[i] = 0.0;
             if (tid == 0) sFail = 0;
             __syncthreads();
-            CS_TIC(0);
 
             // ---- a2 + a3 + a5: left-looking blocked Cholesky with on-the-fly D and fused y = L dW ------
             for (int k0 = 0; k0 < M; k0 += NBP) {
@@ -237,7 +218,6 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                 for (int q = tid; q < (MP - M) * NBP; q += CS_THREADS)          // padding rows M..MP-1
                     tile[TIDX(M - k0 + q / NBP, q % NBP)] = 0.0;
                 __syncthreads();
-                CS_TIC(1);
 
                 // (b) S = D - L[rows, :k0] L[panel, :k0]^T, operands from the TMA ring
                 double acc[CS_MTW][NT][2];
@@ -335,9 +315,7 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                             *tp = dv;
                         }
                     }
-                CS_TIC(2);
                 __syncthreads();
-                CS_TIC(3);
 
                 // (c) diagonal block, warp 0: L_kk (back into the tile) and W = L_kk^-1 (-> winv), one row per lane,
                 //     registers + shuffles (warp_chol.cuh): ~100 cycles per pivot instead of a CTA barrier and a
@@ -382,7 +360,6 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                     }
                 }
                 __syncthreads();
-                CS_TIC(4);
 
                 // (d) rows below the panel: X = S W^T (DMMA, zero blocks of W skipped); panel rows: L_kk.
                 //     X -> Lg (fragment-major) and y += X dW.
@@ -431,7 +408,6 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                 }
                 asm volatile("fence.proxy.async;\n" ::: "memory");           // Lg stores (generic proxy) before later TMA reads
                 __syncthreads();
-                CS_TIC(5);
             }
 
             // ---- a6-a8: semi-implicit rod update, position rebuild, centre of mass -> 0 ----------------
@@ -488,15 +464,10 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                 __syncthreads();
             }
         }
-        CS_TIC(6);
         for (int i = tid; i < M; i += CS_THREADS) rg[i] = sR[i];
         if (tid == 0 && chain_info != 0 && P.info[c] == 0) P.info[c] = chain_info;
         __syncthreads();
     }
-#ifdef CS_PROFILE
-    if (tid == 0 && P.dbg != nullptr)
-        for (int i = 0; i < 8; ++i) P.dbg[blockIdx.x * 8 + i] = prof[i];
-#endif
 }
 
 template <int NT>
@@ -525,9 +496,6 @@ int bdk_chain_step(bd_ctx* ctx, double* r, uint64_t first_step, int n_steps)
     int per_sm = 0;
     BD_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_chain_step<NT>, CS_THREADS, smem));
     if (per_sm < 1) return BD_ERR_CUDA;
-#ifdef CS_PROFILE
-    if (getenv("BD_CS_PER_SM") != nullptr) per_sm = atoi(getenv("BD_CS_PER_SM"));
-#endif
     const int MP = (ctx->M + 7) & ~7;
     ChainStepParams P;
     P.N = ctx->N; P.C = ctx->C;
@@ -536,22 +504,9 @@ int bdk_chain_step(bd_ctx* ctx, double* r, uint64_t first_step, int n_steps)
     for (int i = 0; i < 9; ++i) P.kap[i] = ctx->p.kappa[i];
     P.seed = ctx->p.seed; P.chain0 = ctx->p.chain_id0; P.first_step = first_step;
     P.n_steps = n_steps; P.noise_kind = ctx->p.noise_kind;
-    P.dbg = nullptr;
-#ifdef CS_PROFILE
-    P.dbg = reinterpret_cast<long long*>(ctx->tmp);       // debug builds only: phase cycles land in ctx->tmp
-#endif
     P.r = r; P.scratch = ctx->ws; P.scratch_stride = (int64_t)MP * MP; P.info = ctx->info;
     int grid = ctx->num_sms * per_sm;
     if (grid > ctx->C) grid = ctx->C;
     BD_LAUNCH(ctx, k_chain_step<NT>, dim3(grid), dim3(CS_THREADS), smem, P);
     return 0;
 }
-
-#ifdef CS_PROFILE
-// debug builds only (-DCS_PROFILE): copy the per-CTA phase cycle counters to the host.
-extern "C" int bd_debug_phase_cycles(bd_ctx* ctx, long long* host, int n_ctas)
-{
-    cudaStreamSynchronize(ctx->stream);
-    return (int)cudaMemcpy(host, ctx->tmp, sizeof(long long) * 8 * (size_t)n_ctas, cudaMemcpyDeviceToHost);
-}
-#endif

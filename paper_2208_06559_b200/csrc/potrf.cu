@@ -79,10 +79,11 @@ __global__ void __launch_bounds__(256, 2) k_trsm(double* __restrict__ A_all, int
     extern __shared__ __align__(16) double smem[];
     double* sA = smem;                           // [128][68]
     double* sW = smem + TRSM_ROWS * TRSM_SLD;    // [64][68]
-    const int c = blockIdx.y;
+    const int nrb = (r_hi - r_lo + TRSM_ROWS - 1) / TRSM_ROWS;
+    const int c = blockIdx.x / nrb;                        // chain and row block both on grid.x
     double* A = A_all + (size_t)c * stride;
     const double* W = Winv + (size_t)c * 64 * 64;
-    const int row0 = r_lo + blockIdx.x * TRSM_ROWS;
+    const int row0 = r_lo + (blockIdx.x - c * nrb) * TRSM_ROWS;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, t = lane & 3, wm = warp & 3, wn = warp >> 2;
     {
@@ -138,14 +139,7 @@ __global__ void __launch_bounds__(256, 2) k_trsm(double* __restrict__ A_all, int
 //     load cursor is STAGES-1 k-slabs ahead of the compute cursor and simply moves on to the next tile.
 //   smem rows are padded to BK + 8 doubles: the 16-byte fragment loads (two k-steps each) are conflict free.
 // =================================================================================================
-#ifndef SYRK_BK
-#define SYRK_BK 32
-#define SYRK_STAGES 2
-#endif
-#ifndef SYRK_BN
-#define SYRK_BN 128
-#endif
-constexpr int BM = 128, BN = SYRK_BN, NTW = BN / 16, SYRK_CTAS = (BN == 64) ? 2 : 1, BK = SYRK_BK, STAGES = SYRK_STAGES, SLD = BK + 8;   // SLD % 16 == 8: conflict-free 16-byte fragment loads
+constexpr int BM = 128, BN = 128, NTW = BN / 16, SYRK_CTAS = 1, BK = 32, STAGES = 2, SLD = BK + 8;   // SLD % 16 == 8: conflict-free 16-byte fragment loads
 constexpr int CPR = BK / 2, RPP = 256 / CPR;          // 16-byte chunks per slab row, rows copied per pass of the CTA
 constexpr int SYRK_SMEM = STAGES * (BM + BN) * SLD * (int)sizeof(double);
 
@@ -364,10 +358,8 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
     // outer panel width, from sweeps on B200 (profiles/r01_summary.md): with the recursive panel below, wide outer
     // panels win (c4: 256 -> 0.641, 1024 -> 0.688, 4096 -> 0.695 of peak; c5: 0.686 / 0.769 / 0.781)
     const int NB = (n >= 4096) ? 4096 : 1024;
-    // Outer level: right-looking.  A left-looking outer loop (block column J updated by all finished columns in one
-    // pass, K = J; kept behind `left`) measured equal at c3 / c4 and slower at c5 (0.78 -> 0.75: the K-deep operand
-    // streams of all row blocks no longer share L2).
-    const bool left = false;
+    // Outer level: right-looking.  (A left-looking outer loop -- block column J updated by all finished columns in one
+    // pass, K = J -- measured equal at c3 / c4 and slower at c5, profiles/r01_summary.md.)
     // In-panel factorisation of columns [J0, J1), all rows below included, RECURSIVELY: left half, update of the
     // right half with K = (J1 - J0) / 2, right half.  Against a plain right-looking sweep of 64-column blocks (every
     // block updated once per preceding block, always K = 64, DMMA pipe ~50 % busy) each column block now sees
@@ -380,8 +372,8 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
                 const int nloc = J1 - J0;
                 BD_LAUNCH(ctx, k_potf2, dim3(C), dim3(256), potf2::SMEM_BYTES, A, ld, stride, J0, nloc, info, ctx->Winv);
                 if (J1 < n)
-                    BD_LAUNCH(ctx, k_trsm, dim3((n - J1 + TRSM_ROWS - 1) / TRSM_ROWS, C), dim3(256), trsm_smem, A, ld, stride, J0,
-                              J1, n, ctx->Winv);
+                    BD_LAUNCH(ctx, k_trsm, dim3((unsigned)((int64_t)((n - J1 + TRSM_ROWS - 1) / TRSM_ROWS) * C)), dim3(256), trsm_smem, A, ld,
+                              stride, J0, J1, n, ctx->Winv);
                 return 0;
             }
             const int half = ((J1 - J0) / 2 + BD_NB_INNER - 1) / BD_NB_INNER * BD_NB_INNER;
@@ -394,13 +386,9 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
     } rec{ctx, A, ld, stride, info, n, C, trsm_smem};
     for (int J = 0; J < n; J += NB) {
         const int Jend = (J + NB < n) ? J + NB : n;
-        if (left && J > 0) {
-            int rc = launch_syrk(ctx, A, ld, stride, J, n, Jend, 0, J);
-            if (rc != 0) return rc;
-        }
         int rc = rec.run(J, Jend);
         if (rc != 0) return rc;
-        if (!left && Jend < n) {
+        if (Jend < n) {
             rc = launch_syrk(ctx, A, ld, stride, Jend, n, n, J, Jend - J);
             if (rc != 0) return rc;
         }

@@ -72,11 +72,11 @@ __device__ __forceinline__ void tension(const double* __restrict__ r, int k, dou
     T[0] = c * qx; T[1] = c * qy; T[2] = c * qz;
 }
 
-__global__ void __launch_bounds__(256) k_forces(int N, double K, double b, const double* __restrict__ r_all,
+__global__ void __launch_bounds__(256) k_forces(int N, int nblk, double K, double b, const double* __restrict__ r_all,
                                                 double* __restrict__ T_all, double* __restrict__ F_all)
 {
-    const int c = blockIdx.y;
-    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    const int c = blockIdx.x / nblk;                       // chain and block both on grid.x
+    const int j = (blockIdx.x - c * nblk) * blockDim.x + threadIdx.x;
     if (j > N) return;
     const double* r = r_all + (size_t)c * 3 * (N + 1);
     double Tl[3] = {0, 0, 0}, Tr[3] = {0, 0, 0};
@@ -94,13 +94,13 @@ __global__ void __launch_bounds__(256) k_forces(int N, double K, double b, const
 
 // a4: v_i = sum_j D_ij F_j (Eq. 6 second term, :102) with D_ij recomputed from positions (Eqs. 7-9),
 // so D is never read for the drift.  One warp per bead i, lanes stride over j.
-__global__ void __launch_bounds__(256) k_drift(int N, double hstar, double a_s, double inv_a, double inv_b,
+__global__ void __launch_bounds__(256) k_drift(int N, int nblk, double hstar, double a_s, double inv_a, double inv_b,
                                                const double* __restrict__ r_all, const double* __restrict__ F_all,
                                                double* __restrict__ v_all)
 {
-    const int c = blockIdx.y;
+    const int c = blockIdx.x / nblk;
     const int Nb = N + 1;
-    const int i = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int i = (blockIdx.x - c * nblk) * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (i >= Nb) return;
     const int lane = threadIdx.x & 31;
     const double* r = r_all + (size_t)c * 3 * Nb;
@@ -129,13 +129,13 @@ __global__ void __launch_bounds__(256) k_drift(int N, double hstar, double a_s, 
 //         |Q'_k| = (2 dt K b + |Y_k|)/(2 dt K + 1)         (Eq. 17 :154)
 //         Q'_k = Y_k |Q'_k| / |Y_k|                        (Eq. 15 :144, recipe :156-160)
 //         r'_0 = 0, r'_{k+1} = r'_k + Q'_k, centre of mass -> 0 (reading A8)
-// One CTA per chain.  A chain with info != 0 (failed factorisation) or a non-finite result keeps
-// its positions (reading A10).
+// One CTA per chain.  A chain whose factorisation failed in THIS step (info_step != 0) or whose update is
+// non-finite keeps its positions for this step (reading A10); its first failure code is kept in info_sticky.
 struct UpdParams { double dt, K, b; double kap[9]; };
 
 __global__ void __launch_bounds__(kUpdThreads) k_update(int N, UpdParams P, const double* __restrict__ r_all,
                                                         const double* __restrict__ v_all, const double* __restrict__ y_all,
-                                                        const int32_t* __restrict__ info_in, int32_t* __restrict__ info_out,
+                                                        const int32_t* __restrict__ info_step, int32_t* __restrict__ info_sticky,
                                                         double* __restrict__ tmp_all, double* r_out_all)
 {
     __shared__ double s_buf[96];
@@ -146,7 +146,8 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(int N, UpdParams P, cons
     const double* y = y_all + c * M;
     double* r_out = r_out_all + c * M;
     bool bad = false;
-    const bool skip = (info_in != nullptr && info_in[c] != 0);
+    const int32_t code_in = (info_step != nullptr) ? info_step[c] : 0;       // this step's factorisation failure, if any
+    const bool skip = code_in != 0;
     if (!skip) {
         const double tdk = 2.0 * P.dt * P.K;
         rebuild_positions(N, tmp_all + c * M, r_out, s_buf, bad, [&](int k, double* q) {
@@ -174,7 +175,8 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(int N, UpdParams P, cons
     if (skip || bad) {
         if (r_out != r)
             for (int i = threadIdx.x; i < (int)M; i += blockDim.x) r_out[i] = r[i];
-        if (bad && threadIdx.x == 0 && info_out != nullptr && info_out[c] == 0) info_out[c] = (int32_t)M + 1;
+        // first failure of the chain since the last reset: failing pivot row, or M + 1 for a non-finite update
+        if (threadIdx.x == 0 && info_sticky != nullptr && info_sticky[c] == 0) info_sticky[c] = skip ? code_in : (int32_t)M + 1;
     }
 }
 
@@ -191,19 +193,20 @@ int bdk_drift(bd_ctx* ctx, const double* r, double* T, double* F, double* v)
 {
     double* Fbuf = (F != nullptr) ? F : ctx->F;
     if (T != nullptr || F != nullptr || v != nullptr)
-        BD_LAUNCH(ctx, k_forces, dim3((ctx->Nb + 255) / 256, ctx->C), dim3(256), 0, ctx->N, ctx->p.K, ctx->p.b, r, T, Fbuf);
+        BD_LAUNCH(ctx, k_forces, dim3((unsigned)((int64_t)((ctx->Nb + 255) / 256) * ctx->C)), dim3(256), 0, ctx->N, (ctx->Nb + 255) / 256,
+                  ctx->p.K, ctx->p.b, r, T, Fbuf);
     if (v != nullptr)
-        BD_LAUNCH(ctx, k_drift, dim3((ctx->Nb + 7) / 8, ctx->C), dim3(256), 0, ctx->N, ctx->p.hstar, ctx->p.a / ctx->p.b,
-                  ctx->p.b / ctx->p.a, 1.0 / ctx->p.b, r, Fbuf, v);
+        BD_LAUNCH(ctx, k_drift, dim3((unsigned)((int64_t)((ctx->Nb + 7) / 8) * ctx->C)), dim3(256), 0, ctx->N, (ctx->Nb + 7) / 8, ctx->p.hstar,
+                  ctx->p.a / ctx->p.b, ctx->p.b / ctx->p.a, 1.0 / ctx->p.b, r, Fbuf, v);
     return 0;
 }
 
-int bdk_update(bd_ctx* ctx, const double* r, const double* v, const double* y, const int32_t* info,
-               int32_t* info_out, double* r_out)
+int bdk_update(bd_ctx* ctx, const double* r, const double* v, const double* y, const int32_t* info_step,
+               int32_t* info_sticky, double* r_out)
 {
     UpdParams P;
     P.dt = ctx->p.dt; P.K = ctx->p.K; P.b = ctx->p.b;
     for (int i = 0; i < 9; ++i) P.kap[i] = ctx->p.kappa[i];
-    BD_LAUNCH(ctx, k_update, dim3(ctx->C), dim3(kUpdThreads), 0, ctx->N, P, r, v, y, info, info_out, ctx->tmp, r_out);
+    BD_LAUNCH(ctx, k_update, dim3(ctx->C), dim3(kUpdThreads), 0, ctx->N, P, r, v, y, info_step, info_sticky, ctx->tmp, r_out);
     return 0;
 }

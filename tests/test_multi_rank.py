@@ -55,3 +55,26 @@ def test_shard_bounds():
     assert ensemble.shard(0, 4, 256) == 0 and ensemble.shard(3, 4, 256) == 768
     with pytest.raises(ValueError):
         ensemble.shard(4, 4, 1)
+
+
+def test_bench_gpus_n_starts_n_ranks():
+    """`python bench.py --gpus 2` outside torchrun must start two ranks itself.  Run on the CPU
+    through the reference arm (the oracle; the GPU arm needs CUDA): bench.py re-executes under torch.distributed.run,
+    rank 0 alone prints ONE JSON line, and it refuses to print n_gpus != --gpus, so n_gpus = 2 proves WORLD_SIZE = 2."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--impl", "reference", "--config", "c1",
+                          "--steps", "2", "--warmup", "1"], capture_output=True, text=True, env=env, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["config"]["workload"] == "c1"
+    # inside a torchrun environment whose WORLD_SIZE disagrees with --gpus it refuses
+    env2 = dict(env, WORLD_SIZE="1", RANK="0")
+    bad = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--impl", "reference", "--config", "c1"],
+                         capture_output=True, text=True, env=env2, timeout=600)
+    assert bad.returncode != 0 and "refusing" in (bad.stderr + bad.stdout)
