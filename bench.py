@@ -124,7 +124,7 @@ def _oracle_plan(w: W.Workload):
         chains = min(w.n_chains, 2 * max(cores, 1))
         return {"label": "measured", "chains": chains, "n_rods": w.n_rods, "scale": 1.0, "threads": min(chains, cores)}
     if w.M <= 8000:                                       # c4: one real chain x one step, x C stated as scaled
-        return {"label": "scaled", "chains": 1, "n_rods": w.n_rods, "scale": 1.0 / min(w.n_chains, max(cores, 1)), "threads": 1,
+        return {"label": "scaled", "chains": 1, "n_rods": w.n_rods, "scale": 1.0 / min(w.n_chains, max(cores, 1)), "threads": min(w.n_chains, max(cores, 1)),
                 "concurrent": min(w.n_chains, max(cores, 1))}
     # c5: one step is 9e12 flop (~2 h on one core): a sub-chain of 1001 beads (M = 3003) is stepped for real and the
     # time extrapolated with the M^3 law of the Cholesky (checked against M = 1503 in the same call)
