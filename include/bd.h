@@ -114,6 +114,12 @@ int bd_update(bd_ctx *ctx, const double *r_dev, const double *v_dev, const doubl
  * 1: always staged.  2: always fused (-2 if M is too large).                                        */
 int bd_set_path(bd_ctx *ctx, int32_t path);
 
+/* Which factorisation bd_cholesky / the staged bd_step use.  0 (default): automatic; 1: blocked right-looking
+ * factorisation with a recursive panel, one kernel launch per block operation (k_potf2 / k_trsm / k_syrk);
+ * 2: left-looking tile Cholesky in ONE persistent kernel (TMA-fed DMMA tiles, ticket counter, ready flags).
+ * Both give the same L up to rounding.                                                               */
+int bd_set_cholesky(bd_ctx *ctx, int32_t algo);
+
 /* The whole hot path a0-a8, n_steps times, time steps first_step .. first_step+n_steps-1;
  * r_dev [C][N_b][3] updated in place.  Needs bd_set_workspace.                                   */
 int bd_step(bd_ctx *ctx, double *r_dev, uint64_t first_step, int32_t n_steps);

@@ -28,7 +28,7 @@ class bd_params(C.Structure):
 
 EXPORTS = ("bd_create", "bd_destroy", "bd_workspace_bytes", "bd_set_workspace", "bd_set_flow",
            "bd_init_random_walk", "bd_assemble_hi", "bd_cholesky", "bd_brownian", "bd_noise", "bd_drift",
-           "bd_update", "bd_set_path", "bd_step", "bd_observables", "bd_last_info", "bd_step_host", "bd_profile",
+           "bd_update", "bd_set_path", "bd_set_cholesky", "bd_step", "bd_observables", "bd_last_info", "bd_step_host", "bd_profile",
            "bd_stage_ms", "bd_launch_count", "bd_strerror", "bd_last_error")
 
 _lib = None
@@ -58,6 +58,7 @@ def load_library(path: str | None = None) -> C.CDLL:
     lib.bd_drift.argtypes = [vp, dp, dp, dp, dp]
     lib.bd_update.argtypes = [vp, dp, dp, dp, dp]
     lib.bd_set_path.argtypes = [vp, i32]
+    lib.bd_set_cholesky.argtypes = [vp, i32]
     lib.bd_step.argtypes = [vp, dp, u64, i32]
     lib.bd_observables.argtypes = [vp, dp, dp, dp]
     lib.bd_last_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i32)]
@@ -202,6 +203,10 @@ class BD:
     def set_path(self, path: int):
         """0 auto, 1 staged kernels, 2 fused per-chain kernel."""
         self._check("bd_set_path", self.lib.bd_set_path(self._ctx, int(path)))
+
+    def set_cholesky(self, algo: int):
+        """0 auto, 1 multi-launch blocked factorisation, 2 persistent tile kernel."""
+        self._check("bd_set_cholesky", self.lib.bd_set_cholesky(self._ctx, int(algo)))
 
     def step(self, r, first_step: int = 0, n_steps: int = 1):
         if self._ws is None:

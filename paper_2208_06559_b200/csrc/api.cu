@@ -23,6 +23,13 @@ bool layout_ok(const bd_ctx* ctx, const void* p, int64_t ld, int64_t stride)
 // CUDA error lives in the context (bd_last_error).
 static thread_local cudaError_t tl_create_cuda = cudaSuccess;
 
+// a3 dispatch: the persistent tile kernel unless its O(C M) scratch (128 x 128 inverse blocks) would be unreasonably large
+int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
+{
+    const bool tiles = (ctx->chol_algo == 2) || (ctx->chol_algo == 0 && bdk_potrf_tiles_scratch_bytes(ctx) <= ((size_t)4 << 30));
+    return tiles ? bdk_potrf_tiles(ctx, A, ld, stride, info) : bdk_potrf_launches(ctx, A, ld, stride, info);
+}
+
 extern "C" {
 
 int bd_create(const bd_params* params, void* cuda_stream, bd_ctx** out)
@@ -105,7 +112,8 @@ int bd_destroy(bd_ctx* ctx)
 {
     if (ctx == nullptr) return -1;
     cudaStreamSynchronize(ctx->stream);
-    void* ptrs[] = {ctx->T, ctx->F, ctx->v, ctx->y, ctx->dW, ctx->tmp, ctx->r_own, ctx->info, ctx->info_step, ctx->fail, ctx->obs, ctx->Winv};
+    void* ptrs[] = {ctx->T, ctx->F, ctx->v, ctx->y, ctx->dW, ctx->tmp, ctx->r_own, ctx->info, ctx->info_step, ctx->fail, ctx->obs, ctx->Winv,
+                    ctx->tile_W, ctx->tile_flags};
     for (void* q : ptrs)
         if (q != nullptr) cudaFree(q);
     if (ctx->ev != nullptr) {
@@ -170,6 +178,14 @@ int bd_cholesky(bd_ctx* ctx, double* DL_dev, int64_t ld, int64_t chain_stride, i
     int32_t* info = (info_dev != nullptr) ? info_dev : ctx->info;
     BD_CUDA(ctx, cudaMemsetAsync(info, 0, sizeof(int32_t) * (size_t)ctx->C, ctx->stream));
     return bdk_potrf(ctx, DL_dev, ld, chain_stride, info);
+}
+
+int bd_set_cholesky(bd_ctx* ctx, int32_t algo)
+{
+    if (ctx == nullptr) return -1;
+    if (algo < 0 || algo > 2) return -2;
+    ctx->chol_algo = algo;
+    return 0;
 }
 
 int bd_noise(bd_ctx* ctx, uint64_t step, double* dW_dev)

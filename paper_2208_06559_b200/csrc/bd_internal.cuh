@@ -35,6 +35,15 @@ struct bd_ctx {
     cudaError_t last_cuda;
     int num_sms;
     bool attr_potrf, attr_chain;   // cudaFuncSetAttribute done for this context's device (no process-wide statics)
+    // tile Cholesky (potrf_tiles.cu): inverse diagonal blocks, ready flags (+ ticket counter, error word), tensor maps
+    int32_t chol_algo;             // bd_set_cholesky: 0 auto, 1 multi-launch recursive (potrf.cu), 2 persistent tile kernel
+    double* tile_W;
+    int* tile_flags;
+    int tile_epoch;
+    unsigned tile_ticket_base;
+    const void* tile_mapA_ptr;
+    int64_t tile_mapA_ld, tile_mapA_stride;
+    struct alignas(64) { unsigned char bytes[128]; } tile_maps[2];
 };
 
 #define BD_NB_INNER 64      // width of the diagonal block factored by potf2 (one CTA per chain)
@@ -63,7 +72,10 @@ struct bd_ctx {
 // ---- stage entry points implemented in the .cu files (host side) -------------------------------
 int bdk_init_random_walk(bd_ctx* ctx, double* r, uint64_t init_seed);
 int bdk_assemble(bd_ctx* ctx, const double* r, double* D, int64_t ld, int64_t stride, int full);
-int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info);
+int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info);            // dispatch on chol_algo
+int bdk_potrf_launches(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info);   // potrf.cu
+int bdk_potrf_tiles(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info);      // potrf_tiles.cu
+size_t bdk_potrf_tiles_scratch_bytes(const bd_ctx* ctx);
 int bdk_noise(bd_ctx* ctx, uint64_t step, double* dW);
 int bdk_trmv(bd_ctx* ctx, const double* L, int64_t ld, int64_t stride, const double* dW, double* y);
 int bdk_drift(bd_ctx* ctx, const double* r, double* T, double* F, double* v);

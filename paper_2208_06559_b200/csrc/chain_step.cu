@@ -24,6 +24,7 @@
 #include "bd_internal.cuh"
 #include "block_ops.cuh"
 #include "philox.cuh"
+#include "tma.cuh"
 #include "warp_chol.cuh"
 
 namespace {
@@ -53,41 +54,6 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
                  : "+d"(c0), "+d"(c1)
                  : "d"(a), "d"(b));
 }
-// shared-window (32-bit) address of a shared-memory object, for the mbarrier / TMA instructions
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-// ---- mbarrier + TMA bulk copy (global -> shared) ------------------------------------------------------
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(bar), "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void tma_bulk_g2s(uint32_t dst_smem, const void* src, uint32_t bytes, uint32_t bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(dst_smem),
-                 "l"(src), "r"(bytes), "r"(bar)
-                 : "memory");
-}
-
 template <int NT>
 __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(ChainStepParams P)
 {
@@ -126,7 +92,7 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
     const uint32_t ring_u32 = smem_u32(ring);
     if (tid == 0) {
         for (int s = 0; s < CS_STAGES; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, CS_WARPS); }
-        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        mbar_fence_init();
     }
     __syncthreads();
     uint32_t git = 0;                      // global k-group counter (ring position / barrier parity), same in all threads
@@ -406,7 +372,7 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                     part += __shfl_xor_sync(0xffffffffu, part, 2);
                     if (t == 0) sY[8 * mt + g] += part;
                 }
-                asm volatile("fence.proxy.async;\n" ::: "memory");           // Lg stores (generic proxy) before later TMA reads
+                fence_proxy_async();                                          // Lg stores (generic proxy) before later TMA reads
                 __syncthreads();
             }
 

@@ -43,6 +43,35 @@ __device__ __forceinline__ void gemm32(const double* __restrict__ X, const doubl
     }
 }
 
+// The same for 64 x 64 operands (the 128 x 128 diagonal tile of the tile kernel, split 64 + 64): warp w owns output rows
+// 16 (w & 3) .. +15 and columns 32 (w >> 2) .. +31 (2 x 4 accumulators, 16 k-steps).  Lane (g, t) ends up with
+// out[mm][nn][0..1] = element (row 16 (w & 3) + 8 mm + g, column 32 (w >> 2) + 8 nn + 2 t + {0, 1}).
+__device__ __forceinline__ void gemm64(const double* __restrict__ X, const double* __restrict__ Y, bool yt, int warp, int lane,
+                                       double (&out)[2][4][2])
+{
+    const int g = lane >> 2, t = lane & 3, r0 = 16 * (warp & 3), c0 = 32 * (warp >> 2);
+#pragma unroll
+    for (int mm = 0; mm < 2; ++mm)
+#pragma unroll
+        for (int nn = 0; nn < 4; ++nn) out[mm][nn][0] = out[mm][nn][1] = 0.0;
+#pragma unroll 4
+    for (int ks = 0; ks < 16; ++ks) {
+        double a[2];
+#pragma unroll
+        for (int mm = 0; mm < 2; ++mm) a[mm] = X[(r0 + 8 * mm + g) * SLDP + 4 * ks + t];
+#pragma unroll
+        for (int nn = 0; nn < 4; ++nn) {
+            const int j = c0 + 8 * nn + g, p = 4 * ks + t;
+            const double b = yt ? Y[p * SLDP + j] : Y[j * SLDP + p];
+#pragma unroll
+            for (int mm = 0; mm < 2; ++mm)
+                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                             : "+d"(out[mm][nn][0]), "+d"(out[mm][nn][1])
+                             : "d"(a[mm]), "d"(b));
+        }
+    }
+}
+
 // rows / columns o .. o+31 of the working copy: warp 0 factors (L back into S, 1 / L_kk into s_rinv), warp 1 forms the
 // inverse of that 32 x 32 factor in Wm, 4 pivots behind (named barriers 1..8).  Called from ONE place (a loop over the two
 // halves): the fully unrolled pivot loops are ~1700 straight-line instructions, and a second inlined copy ran 4x slower.
@@ -64,63 +93,41 @@ __device__ __forceinline__ void factor_half(double* __restrict__ S, double* __re
     }
 }
 
-constexpr int SMEM_BYTES = (2 * 64 * SLDP + 128) * (int)sizeof(double);
-
-__global__ void __launch_bounds__(256) k_potf2(double* __restrict__ A_all, int64_t ld, int64_t stride, int j0, int nloc,
-                                               int32_t* __restrict__ info, double* __restrict__ Winv)
+// Factor AND invert one 64 x 64 block held in shared memory: on entry S holds the lower triangle of the block (row stride
+// SLDP), Wm is zero; on exit S = L (lower, zeros above the diagonal) and Wm = L^-1.  nh = 2 does both 32-column halves
+// (steps 1-5 of the header), nh = 1 only the first (blocks of <= 32 rows, identity padded).  All 8 warps of the calling
+// group take part; `sync()` is the barrier of that group (the whole CTA in k_potf2, a named barrier in the tile kernel).
+// row0 = 0-based global row of the block (for the failing-pivot report in *sFail, 1-based).
+//
+// ONE copy of the factor / inverse code, run once per half: a second inlined copy (64 KB further into the kernel) ran 4x
+// slower than the first one (22 k against 5.5 k cycles for the same 32 pivots -- instruction fetch of ~1700 straight-line
+// instructions that are cold at every launch), a loop re-runs warm instructions.
+template <class Sync>
+__device__ __forceinline__ void block64(double* __restrict__ S, double* __restrict__ Wm, double* __restrict__ sCol,
+                                        double* __restrict__ sRinv, const int nh, const int lane, const int warp, const int row0,
+                                        int* sFail, Sync&& sync)
 {
-    extern __shared__ __align__(16) double sm[];
-    double* S = sm;                       // [64][SLDP] the block, then L (lower, zeros above the diagonal)
-    double* Wm = S + 64 * SLDP;           // [64][SLDP] W = L^-1
-    double* sCol = Wm + 64 * SLDP;        // [64] column broadcast buffer of warp_chol
-    double* sRinv = sCol + 64;            // [64] 1 / L_kk
-    __shared__ int sFail;
-    const int c = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    double* A = A_all + (size_t)c * stride + (size_t)j0 * ld + j0;
-    {
-        double v[16];                                              // all 16 loads of a thread in flight at once
-#pragma unroll
-        for (int it = 0; it < 16; ++it) {
-            const int idx = tid + 256 * it, i = idx >> 6, j = idx & 63;
-            v[it] = (i == j) ? 1.0 : 0.0;                          // identity padding for a ragged block
-            if (i < nloc && j <= i) v[it] = A[(size_t)i * ld + j];
-        }
-#pragma unroll
-        for (int it = 0; it < 16; ++it) {
-            const int idx = tid + 256 * it, i = idx >> 6, j = idx & 63;
-            S[i * SLDP + j] = (j <= i) ? v[it] : 0.0;
-            Wm[i * SLDP + j] = 0.0;
-        }
-    }
-    if (tid == 0) sFail = 0;
-    __syncthreads();
-
     const int oi = 8 * (warp & 3) + (lane >> 2), oj = 16 * (warp >> 2) + 2 * (lane & 3);   // this lane's outputs: (oi, oj + 8 nn + {0, 1})
     double out[2][2];
-
-    // ONE copy of the factor / inverse code, run once per half: a second inlined copy (64 KB further into the kernel)
-    // ran 4x slower than the first one (22 k against 5.5 k cycles for the same 32 pivots -- instruction fetch of
-    // ~1700 straight-line instructions that are cold at every launch), a loop re-runs warm instructions.
-    const int nh = (nloc > HB) ? 2 : 1;
 #pragma unroll 1
     for (int hh = 0; hh < nh; ++hh) {
-        factor_half(S, Wm, sCol, sRinv, hh * HB, lane, warp, j0, &sFail);
-        __syncthreads();
+        factor_half(S, Wm, sCol, sRinv, hh * HB, lane, warp, row0, sFail);
+        sync();
         if (hh == 0 && nh == 2) {
             gemm32(S + HB * SLDP, Wm, false, warp, lane, out);         // L21 = A21 W11^T
-            __syncthreads();
+            sync();
 #pragma unroll
             for (int nn = 0; nn < 2; ++nn)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) S[(HB + oi) * SLDP + oj + 8 * nn + e] = out[nn][e];
-            __syncthreads();
+            sync();
             gemm32(S + HB * SLDP, S + HB * SLDP, false, warp, lane, out);   // A22 -= L21 L21^T (lower part)
 #pragma unroll
             for (int nn = 0; nn < 2; ++nn)
 #pragma unroll
                 for (int e = 0; e < 2; ++e)
                     if (oj + 8 * nn + e <= oi) S[(HB + oi) * SLDP + HB + oj + 8 * nn + e] -= out[nn][e];
-            __syncthreads();
+            sync();
         }
     }
     if (nh == 2) {
@@ -129,23 +136,14 @@ __global__ void __launch_bounds__(256) k_potf2(double* __restrict__ A_all, int64
         for (int nn = 0; nn < 2; ++nn)
 #pragma unroll
             for (int e = 0; e < 2; ++e) Wm[(HB + oi) * SLDP + oj + 8 * nn + e] = out[nn][e];
-        __syncthreads();
+        sync();
         gemm32(Wm + HB * SLDP + HB, Wm + HB * SLDP, true, warp, lane, out);   // W21 = -W22 T
-        __syncthreads();
+        sync();
 #pragma unroll
         for (int nn = 0; nn < 2; ++nn)
 #pragma unroll
             for (int e = 0; e < 2; ++e) Wm[(HB + oi) * SLDP + oj + 8 * nn + e] = -out[nn][e];
-        __syncthreads();
-    }
-    if (tid == 0 && sFail != 0 && info != nullptr && info[c] == 0) info[c] = sFail;
-    for (int idx = tid; idx < 64 * 64; idx += 256) {
-        const int r = idx >> 6, j = idx & 63;
-        if (r < nloc && j <= r) A[(size_t)r * ld + j] = S[r * SLDP + j];
-    }
-    if (Winv != nullptr && nloc == 64) {
-        double* W = Winv + (size_t)c * 64 * 64;
-        for (int idx = tid; idx < 64 * 64; idx += 256) W[idx] = Wm[(idx >> 6) * SLDP + (idx & 63)];
+        sync();
     }
 }
 

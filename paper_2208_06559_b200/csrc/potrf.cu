@@ -36,8 +36,53 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 }
 
 
-// k_potf2 (diagonal blocks): potf2_blocked.cuh
-using potf2::k_potf2;
+// k_potf2 (64 x 64 diagonal blocks, one CTA per chain): the block is factored and inverted in shared memory by
+// potf2::block64 (potf2_blocked.cuh)
+constexpr int POTF2_SMEM = (2 * 64 * potf2::SLDP + 128) * (int)sizeof(double);
+
+__global__ void __launch_bounds__(256) k_potf2(double* __restrict__ A_all, int64_t ld, int64_t stride, int j0, int nloc,
+                                               int32_t* __restrict__ info, double* __restrict__ Winv)
+{
+    using namespace potf2;
+    extern __shared__ __align__(16) double sm[];
+    double* S = sm;                       // [64][SLDP] the block, then L (lower, zeros above the diagonal)
+    double* Wm = S + 64 * SLDP;           // [64][SLDP] W = L^-1
+    double* sCol = Wm + 64 * SLDP;        // [64] column broadcast buffer of warp_chol
+    double* sRinv = sCol + 64;            // [64] 1 / L_kk
+    __shared__ int sFail;
+    const int c = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    double* A = A_all + (size_t)c * stride + (size_t)j0 * ld + j0;
+    {
+        double v[16];                                              // all 16 loads of a thread in flight at once
+#pragma unroll
+        for (int it = 0; it < 16; ++it) {
+            const int idx = tid + 256 * it, i = idx >> 6, j = idx & 63;
+            v[it] = (i == j) ? 1.0 : 0.0;                          // identity padding for a ragged block
+            if (i < nloc && j <= i) v[it] = A[(size_t)i * ld + j];
+        }
+#pragma unroll
+        for (int it = 0; it < 16; ++it) {
+            const int idx = tid + 256 * it, i = idx >> 6, j = idx & 63;
+            S[i * SLDP + j] = (j <= i) ? v[it] : 0.0;
+            Wm[i * SLDP + j] = 0.0;
+        }
+    }
+    if (tid == 0) sFail = 0;
+    __syncthreads();
+
+    block64(S, Wm, sCol, sRinv, (nloc > HB) ? 2 : 1, lane, warp, j0, &sFail, [] { __syncthreads(); });
+
+    if (tid == 0 && sFail != 0 && info != nullptr && info[c] == 0) info[c] = sFail;
+    for (int idx = tid; idx < 64 * 64; idx += 256) {
+        const int r = idx >> 6, j = idx & 63;
+        if (r < nloc && j <= r) A[(size_t)r * ld + j] = S[r * SLDP + j];
+    }
+    if (Winv != nullptr && nloc == 64) {
+        double* W = Winv + (size_t)c * 64 * 64;
+        for (int idx = tid; idx < 64 * 64; idx += 256) W[idx] = Wm[(idx >> 6) * SLDP + (idx & 63)];
+    }
+}
+
 
 // =================================================================================================
 // k_trsm: rows gi in [r_lo, r_hi) of the panel at columns [j0, j0+64): X L^T = A  <=>  X = A W^T with
@@ -345,13 +390,13 @@ int launch_syrk(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int lo, int 
 
 }  // namespace
 
-int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
+int bdk_potrf_launches(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
 {
     const int trsm_smem = TRSM_SMEM;
     if (!ctx->attr_potrf) {
         BD_CUDA(ctx, cudaFuncSetAttribute(k_syrk, cudaFuncAttributeMaxDynamicSharedMemorySize, SYRK_SMEM));
         BD_CUDA(ctx, cudaFuncSetAttribute(k_trsm, cudaFuncAttributeMaxDynamicSharedMemorySize, trsm_smem));
-        BD_CUDA(ctx, cudaFuncSetAttribute(k_potf2, cudaFuncAttributeMaxDynamicSharedMemorySize, potf2::SMEM_BYTES));
+        BD_CUDA(ctx, cudaFuncSetAttribute(k_potf2, cudaFuncAttributeMaxDynamicSharedMemorySize, POTF2_SMEM));
         ctx->attr_potrf = true;
     }
     const int n = ctx->M, C = ctx->C;
@@ -370,7 +415,7 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
         {
             if (J1 - J0 <= BD_NB_INNER) {
                 const int nloc = J1 - J0;
-                BD_LAUNCH(ctx, k_potf2, dim3(C), dim3(256), potf2::SMEM_BYTES, A, ld, stride, J0, nloc, info, ctx->Winv);
+                BD_LAUNCH(ctx, k_potf2, dim3(C), dim3(256), POTF2_SMEM, A, ld, stride, J0, nloc, info, ctx->Winv);
                 if (J1 < n)
                     BD_LAUNCH(ctx, k_trsm, dim3((unsigned)((int64_t)((n - J1 + TRSM_ROWS - 1) / TRSM_ROWS) * C)), dim3(256), trsm_smem, A, ld,
                               stride, J0, J1, n, ctx->Winv);

@@ -1,0 +1,496 @@
+// potrf_tiles.cu -- a3: in-place FP64 Cholesky D = L L^T of the lower triangle (Eq. 10), batched over
+// chains, as ONE persistent kernel per factorisation: a LEFT-LOOKING TILE Cholesky driven by a ticket counter and
+// per-tile ready flags (the paper calls cusolverDnDpotrf once per chain and step, :172).
+//
+//   The matrix is cut into 128 x 128 tiles (i, j), i >= j.  Tile (i, j) is owned by one CTA from start to finish:
+//     acc = -D_ij + sum_{k < 128 j} L[i-rows][k] L[j-rows][k]       K-deep FP64 tensor-core (DMMA m8n8k4) loop, the
+//                                                                    C tile never leaves the accumulators
+//     i > j:  S = -acc;  L_ij = S W_j^T  with W_j = L_jj^-1          a second, 128-deep pass through the same pipeline
+//     i = j:  L_jj = chol(S), W_j = L_jj^-1                          in shared memory (potf2_blocked.cuh, 64 + 64)
+//   Tickets are handed out column by column (j outer, then chain, then i); a tile waits (ld.acquire on the ready flag
+//   of the tiles it reads) only for tiles with SMALLER tickets, which running CTAs own, so the schedule cannot
+//   deadlock and needs no co-residency.  Later columns start while the diagonal block of the current one is still being
+//   factored: the lookahead that the multi-launch version (potrf.cu) does not have, and one launch instead of
+//   ~6 M / 64 of them.
+//
+//   Operands come through TMA: a 3-D tensor map over the row-major storage (column, row, chain), boxes of 128 rows x 16
+//   columns (= 128 B rows, SWIZZLE_128B), two boxes per operand and stage, 3-stage ring of 64 KB stages with full /
+//   empty mbarriers; one producer thread (warp 8; its warpgroup gives its registers away with setmaxnreg) issues the copies, 8 consumer warps (4 x 2, warp tile 32 x 64) never
+//   meet at a CTA barrier inside the K loop.  Rows beyond M are zero-filled by the TMA unit (ragged last tile).
+//   SYRK/GEMM symmetry: A and B fragments index the k dimension identically, so a lane may read ANY k of the slab as
+//   long as both operands use the same map: lane (g, t) reads 16-byte chunk (2 t + j) ^ g of row g (j = 0, 1), which
+//   is conflict free under the 128-byte swizzle (the 8 lanes of a quarter-warp hit 8 distinct chunks).
+#include <cuda.h>          // CUtensorMap and its enums only; cuTensorMapEncodeTiled is fetched through the runtime (no -lcuda)
+
+#include "bd_internal.cuh"
+#include "potf2_blocked.cuh"
+#include "tma.cuh"
+
+namespace {
+
+constexpr int TB = 128;                       // tile size
+constexpr int BOXK = 16;                      // columns per TMA box (128 bytes = the swizzle span)
+constexpr int BK = 32;                        // columns per ring stage (two boxes per operand)
+constexpr int SPB = TB / BK;                  // stages per 128-column block
+constexpr int STAGES = 3;
+constexpr int BOX_BYTES = TB * BOXK * 8;      // 16 KB
+constexpr int STAGE_BYTES = 4 * BOX_BYTES;    // A box 0, A box 1, B box 0, B box 1
+constexpr int NCONS = 256;                    // consumer threads (8 warps)
+constexpr int NTHREADS = NCONS + 128;         // + the producer warpgroup (one lane of it works; setmaxnreg is per warpgroup)
+constexpr int REGS_PRODUCER = 40, REGS_CONSUMER = 232;   // 8 x 32 x 232 + 4 x 32 x 40 = 64512 <= 65536 registers
+constexpr int RING_BYTES = STAGES * STAGE_BYTES;
+constexpr int TILE_SMEM = RING_BYTES + 1024;  // + slack to align the ring to 1024 B (SWIZZLE_128B atom)
+constexpr long long SPIN_LIMIT = 8000000000LL;   // ~4 s of SM clocks: a lost dependency flags an error instead of hanging
+
+struct TileArgs {
+    double* A;
+    int64_t ld, stride;
+    int M, C, T;
+    double* Wbuf;            // [C][T][128][128] inverse diagonal blocks
+    int* flags;              // [C][T][T]: == epoch when tile (i, j) of chain c is final
+    int epoch;
+    unsigned* ticket;
+    unsigned ticket_base, total;
+    int32_t* info;           // [C]
+    int* err;                // set when a dependency wait timed out
+};
+
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+__device__ __forceinline__ void cons_sync() { asm volatile("bar.sync 9, 256;\n" ::: "memory"); }   // the 8 consumer warps
+
+__device__ __forceinline__ void wait_flag(const int* f, int epoch, int* err)
+{
+    if (ld_acquire_gpu(f) == epoch) return;
+    const long long t0 = clock64();
+    while (ld_acquire_gpu(f) != epoch) {
+        __nanosleep(100);
+        if (clock64() - t0 > SPIN_LIMIT) { atomicExch(err, 1); return; }
+        if (*reinterpret_cast<volatile int*>(err) != 0) return;
+    }
+}
+
+// ticket -> (column j, chain c, row i): columns in order, inside a column chain by chain, inside a chain i = j .. T-1
+__device__ __forceinline__ void decode_ticket(unsigned tk, int C, int T, int& j, int& c, int& i)
+{
+    const long long q = (long long)(tk / (unsigned)C);         // tiles of one chain in the columns before: j T - j (j-1) / 2 <= q
+    const double b = 2.0 * T + 1.0;
+    int jj = (int)((b - sqrt(fmax(b * b - 8.0 * (double)q, 0.0))) * 0.5);
+    jj = max(0, min(jj, T - 1));
+    auto before = [&](int x) { return (long long)x * T - (long long)x * (x - 1) / 2; };
+    while (jj + 1 < T && before(jj + 1) * C <= (long long)tk) ++jj;
+    while (jj > 0 && before(jj) * C > (long long)tk) --jj;
+    const long long rem = (long long)tk - before(jj) * C;
+    const int w = T - jj;
+    j = jj;
+    c = (int)(rem / w);
+    i = jj + (int)(rem - (long long)c * w);
+}
+
+__global__ void __launch_bounds__(NTHREADS, 1) k_potrf_tiles(const __grid_constant__ CUtensorMap tmA,
+                                                             const __grid_constant__ CUtensorMap tmW, const TileArgs a)
+{
+    extern __shared__ uint8_t smem_raw[];
+    __shared__ __align__(8) uint64_t sBar[2 * STAGES + 1];     // full[0..S), empty[S..2S), S-stored
+    __shared__ unsigned sTicket;
+    __shared__ int sFail;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm = warp & 3, wn = (warp >> 2) & 1;
+    const int g = lane >> 2, t = lane & 3;
+    const uint32_t ring = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    uint8_t* ring_g = smem_raw + (ring - smem_u32(smem_raw));
+    const uint32_t bar_full = smem_u32(&sBar[0]), bar_empty = smem_u32(&sBar[STAGES]), bar_s = smem_u32(&sBar[2 * STAGES]);
+
+    if (tid == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, NCONS / 32); }
+        mbar_init(bar_s, NCONS);
+        mbar_fence_init();
+        sTicket = atomicAdd(a.ticket, 1u) - a.ticket_base;
+    }
+    __syncthreads();
+
+    uint32_t git = 0;          // ring stages consumed so far (same value in every thread)
+    uint32_t sphase = 0;       // uses of the S-stored barrier so far
+    const int M = a.M, T = a.T;
+    const int64_t ld = a.ld;
+    // fragment addressing inside a 128 x 16 box: row r at r * 128 bytes, logical 16-byte chunk q at (q ^ (r & 7)) * 16
+    const int xo0 = ((2 * t) ^ g) * 16, xo1 = ((2 * t + 1) ^ g) * 16;
+    const int offA = (wm * 32 + g) * 128, offB = (wn * 64 + g) * 128;
+
+    // Register budget: 384 threads cap the kernel at 168 registers per thread (each of the 4 sub-partitions holds 3
+    // warps); the producer warpgroup hands its share to the 8 consumer warps (64 accumulators + fragments) with
+    // setmaxnreg.  The two roles run SEPARATE tile loops from here to the end of the kernel (ptxas allocates registers per
+    // region; after a common merge point it would have to assume the smaller budget) and meet at the two CTA barriers
+    // that end every tile.
+    if (warp >= NCONS / 32) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(REGS_PRODUCER));
+        while (true) {
+            const unsigned tk = sTicket;
+            if (tk >= a.total) break;
+            int i, j, c;
+            decode_ticket(tk, a.C, T, j, c, i);
+            const bool diag = (i == j);
+            const int KT = j * SPB;                       // ring stages of the K loop
+            const int KE = diag ? 0 : SPB;                // ring stages of the S W^T pass
+            int* flags_c = a.flags + (size_t)c * T * T;
+            const int tm0 = i * TB, tn0 = j * TB;
+            // ============================== producer: one thread feeds the ring ==============================
+            if (warp == NCONS / 32 && lane == 0) {
+                auto acquire_slot = [&](uint32_t G) {
+                    const uint32_t sl = G % STAGES;
+                    if (G >= STAGES) mbar_wait(bar_empty + 8 * sl, ((G / STAGES) - 1) & 1);
+                    return sl;
+                };
+                int ready = 0;                        // 128-column blocks known to be final in rows i and j
+                if (j > 0 && ld_acquire_gpu(flags_c + (size_t)i * T + j - 1) == a.epoch &&
+                    ld_acquire_gpu(flags_c + (size_t)j * T + j - 1) == a.epoch) {
+                    ready = j;                        // tile (., j-1) final => every (., k < j-1) it read is final too
+                    fence_proxy_async();
+                }
+                for (int kb = 0; kb < j; ++kb) {
+                    if (kb >= ready) {
+                        wait_flag(flags_c + (size_t)i * T + kb, a.epoch, a.err);
+                        if (!diag) wait_flag(flags_c + (size_t)j * T + kb, a.epoch, a.err);
+                        fence_proxy_async();          // the acquired tiles are read through the async proxy (TMA)
+                    }
+                    for (int s4 = 0; s4 < SPB; ++s4) {
+                        const uint32_t G = git + kb * SPB + s4, sl = acquire_slot(G);
+                        const uint32_t dst = ring + sl * STAGE_BYTES, fb = bar_full + 8 * sl;
+                        const int k0 = kb * TB + s4 * BK;
+                        mbar_expect_tx(fb, diag ? 2 * BOX_BYTES : 4 * BOX_BYTES);
+                        tma_tile_3d(dst, &tmA, k0, tm0, c, fb);
+                        tma_tile_3d(dst + BOX_BYTES, &tmA, k0 + BOXK, tm0, c, fb);
+                        if (!diag) {
+                            tma_tile_3d(dst + 2 * BOX_BYTES, &tmA, k0, tn0, c, fb);
+                            tma_tile_3d(dst + 3 * BOX_BYTES, &tmA, k0 + BOXK, tn0, c, fb);
+                        }
+                    }
+                }
+                if (!diag) {
+                    mbar_wait(bar_s, sphase & 1);     // the consumers have stored S (generic proxy) ...
+                    fence_proxy_async();              // ... which is now read back through TMA
+                    wait_flag(flags_c + (size_t)j * T + j, a.epoch, a.err);     // L_jj and W_j are final
+                    fence_proxy_async();
+                    for (int s4 = 0; s4 < SPB; ++s4) {
+                        const uint32_t G = git + KT + s4, sl = acquire_slot(G);
+                        const uint32_t dst = ring + sl * STAGE_BYTES, fb = bar_full + 8 * sl;
+                        mbar_expect_tx(fb, 4 * BOX_BYTES);
+                        tma_tile_3d(dst, &tmA, tn0 + s4 * BK, tm0, c, fb);                          // S[rows i][p]
+                        tma_tile_3d(dst + BOX_BYTES, &tmA, tn0 + s4 * BK + BOXK, tm0, c, fb);
+                        tma_tile_2d(dst + 2 * BOX_BYTES, &tmW, s4 * BK, (c * T + j) * TB, fb);      // W_j[cc][p]
+                        tma_tile_2d(dst + 3 * BOX_BYTES, &tmW, s4 * BK + BOXK, (c * T + j) * TB, fb);
+                    }
+                }
+            }
+            __syncwarp();                             // lanes 1..31 wait here for the producer lane
+            git += (uint32_t)(KT + KE);
+            if (!diag) sphase += 1;
+            __syncthreads();                          // tile finished (the consumers may have used the ring as scratch)
+            __syncthreads();                          // next ticket published
+        }
+    } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(REGS_CONSUMER));
+        while (true) {
+            const unsigned tk = sTicket;
+            if (tk >= a.total) break;
+            int i, j, c;
+            decode_ticket(tk, a.C, T, j, c, i);
+            const bool diag = (i == j);
+            const int KT = j * SPB;
+            const int KE = diag ? 0 : SPB;
+            double* A = a.A + (size_t)c * a.stride;
+            int* flags_c = a.flags + (size_t)c * T * T;
+            const int tm0 = i * TB, tn0 = j * TB;
+            // ============================== consumers: 8 warps, warp tile 32 x 64 =============================
+            // this warp's 32 x 64 block lies entirely above the diagonal of a diagonal tile -> no arithmetic
+            const bool warp_active = !diag || (wn * 64 <= wm * 32 + 31);
+            double acc[4][8][2];
+            if (warp_active) {
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt) {
+                    const int gi = tm0 + wm * 32 + mt * 8 + g;
+                    const double* crow = A + (size_t)gi * ld;
+#pragma unroll
+                    for (int nt = 0; nt < 8; ++nt) {
+                        const int gj = tn0 + wn * 64 + nt * 8 + 2 * t;
+                        double c0 = 0.0, c1 = 0.0;
+                        if (gi < M) {
+                            if (gj + 1 <= gi) {
+                                const double2 cv = *reinterpret_cast<const double2*>(crow + gj);
+                                c0 = cv.x; c1 = cv.y;
+                            } else if (gj <= gi) {
+                                c0 = crow[gj];
+                            }
+                        }
+                        acc[mt][nt][0] = -c0;
+                        acc[mt][nt][1] = -c1;
+                    }
+                }
+            }
+            // one ring stage: 2 boxes x 2 chunk pairs x (12 LDS.128 + 64 DMMA) per warp
+            auto compute_stage = [&](uint32_t sl, bool b_is_a) {
+                const uint8_t* sa = ring_g + sl * STAGE_BYTES + offA;
+                const uint8_t* sb = ring_g + sl * STAGE_BYTES + (b_is_a ? 0 : 2 * BOX_BYTES) + offB;
+#pragma unroll
+                for (int bx = 0; bx < 2; ++bx) {
+#pragma unroll
+                    for (int jj = 0; jj < 2; ++jj) {
+                        const int xo = jj ? xo1 : xo0;
+                        double2 af[4], bf[8];
+#pragma unroll
+                        for (int mt = 0; mt < 4; ++mt) af[mt] = *reinterpret_cast<const double2*>(sa + bx * BOX_BYTES + mt * 1024 + xo);
+#pragma unroll
+                        for (int nt = 0; nt < 8; ++nt) bf[nt] = *reinterpret_cast<const double2*>(sb + bx * BOX_BYTES + nt * 1024 + xo);
+#pragma unroll
+                        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                            for (int nt = 0; nt < 8; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], af[mt].x, bf[nt].x);
+#pragma unroll
+                        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                            for (int nt = 0; nt < 8; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], af[mt].y, bf[nt].y);
+                    }
+                }
+            };
+            for (int kt = 0; kt < KT; ++kt) {
+                const uint32_t G = git + kt, sl = G % STAGES;
+                mbar_wait(bar_full + 8 * sl, (G / STAGES) & 1);
+                if (warp_active) compute_stage(sl, diag);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_empty + 8 * sl);
+            }
+
+            if (!diag) {
+                // ---- S = D_ij - sum  ->  global (in place), read back as the A operand of  L_ij = S W_j^T ----
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt) {
+                    const int gi = tm0 + wm * 32 + mt * 8 + g;
+                    if (gi >= M) continue;
+                    double* crow = A + (size_t)gi * ld;
+#pragma unroll
+                    for (int nt = 0; nt < 8; ++nt) {
+                        const int gj = tn0 + wn * 64 + nt * 8 + 2 * t;           // gj + 1 < tn0 + 128 <= tm0 <= gi
+                        *reinterpret_cast<double2*>(crow + gj) = make_double2(-acc[mt][nt][0], -acc[mt][nt][1]);
+                    }
+                }
+                fence_proxy_async();
+                mbar_arrive(bar_s);
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                    for (int nt = 0; nt < 8; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
+                // X[r][cc] = sum_{p <= cc} S[r][p] W[cc][p]: columns 0..63 (wn = 0) need p < 64 only -> stages 0, 1
+                for (int s4 = 0; s4 < SPB; ++s4) {
+                    const uint32_t G = git + KT + s4, sl = G % STAGES;
+                    mbar_wait(bar_full + 8 * sl, (G / STAGES) & 1);
+                    if (wn == 1 || s4 < SPB / 2) compute_stage(sl, false);
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar_empty + 8 * sl);
+                }
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt) {
+                    const int gi = tm0 + wm * 32 + mt * 8 + g;
+                    if (gi >= M) continue;
+                    double* crow = A + (size_t)gi * ld;
+#pragma unroll
+                    for (int nt = 0; nt < 8; ++nt) {
+                        const int gj = tn0 + wn * 64 + nt * 8 + 2 * t;
+                        *reinterpret_cast<double2*>(crow + gj) = make_double2(acc[mt][nt][0], acc[mt][nt][1]);
+                    }
+                }
+                __threadfence();
+                fence_proxy_async();
+                cons_sync();
+                if (tid == 0) st_release_gpu(flags_c + (size_t)i * T + j, a.epoch);
+            } else {
+                // ---- diagonal tile: S -> shared memory, L_jj = chol(S) and W_j = L_jj^-1 as 64 + 64 -------------
+                cons_sync();                                          // every warp is done with the ring
+                double* S11 = reinterpret_cast<double*>(ring_g);
+                double* S21 = S11 + 64 * potf2::SLDP;
+                double* S22 = S21 + 64 * potf2::SLDP;
+                double* W11 = S22 + 64 * potf2::SLDP;
+                double* W22 = W11 + 64 * potf2::SLDP;
+                double* sCol = W22 + 64 * potf2::SLDP;
+                double* sRinv = sCol + 64;
+                const int nloc = min(TB, M - tn0);                    // rows / columns of the block that exist
+                for (int idx = tid; idx < 64 * potf2::SLDP; idx += NCONS) { W11[idx] = 0.0; W22[idx] = 0.0; }
+                if (warp_active) {
+#pragma unroll
+                    for (int mt = 0; mt < 4; ++mt) {
+                        const int R = wm * 32 + mt * 8 + g;
+#pragma unroll
+                        for (int nt = 0; nt < 8; ++nt)
+#pragma unroll
+                            for (int e = 0; e < 2; ++e) {
+                                const int Cc = wn * 64 + nt * 8 + 2 * t + e;
+                                double v = (Cc <= R) ? -acc[mt][nt][e] : 0.0;
+                                if (R >= nloc || Cc >= nloc) v = (R == Cc) ? 1.0 : 0.0;       // identity padding (ragged tile)
+                                double* dst = (R < 64) ? S11 + R * potf2::SLDP + Cc
+                                                       : (Cc < 64 ? S21 + (R - 64) * potf2::SLDP + Cc : S22 + (R - 64) * potf2::SLDP + (Cc - 64));
+                                if (R >= 64 || Cc < 64) *dst = v;
+                            }
+                    }
+                }
+                if (tid == 0) sFail = 0;
+                cons_sync();
+                const int g64r = 16 * (warp & 3), g64c = 32 * (warp >> 2);     // gemm64 output block of this warp
+                double o[2][4][2];
+#pragma unroll 1
+                for (int hh = 0; hh < 2; ++hh) {
+                    double* Sb = hh ? S22 : S11;
+                    double* Wb = hh ? W22 : W11;
+                    const int nrem = nloc - 64 * hh;
+                    potf2::block64(Sb, Wb, sCol, sRinv, (nrem > potf2::HB) ? 2 : 1, lane, warp, tn0 + 64 * hh, &sFail, [] { cons_sync(); });
+                    if (hh == 0) {
+                        potf2::gemm64(S21, W11, false, warp, lane, o);             // L21 = S21 W11^T
+                        cons_sync();
+#pragma unroll
+                        for (int mm = 0; mm < 2; ++mm)
+#pragma unroll
+                            for (int nn = 0; nn < 4; ++nn) {
+                                const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t;
+                                S21[r * potf2::SLDP + cc] = o[mm][nn][0];
+                                S21[r * potf2::SLDP + cc + 1] = o[mm][nn][1];
+                                const int gi = tn0 + 64 + r;
+                                if (gi < M) *reinterpret_cast<double2*>(A + (size_t)gi * ld + tn0 + cc) = make_double2(o[mm][nn][0], o[mm][nn][1]);
+                            }
+                        cons_sync();
+                        potf2::gemm64(S21, S21, false, warp, lane, o);             // S22 -= L21 L21^T (lower part)
+#pragma unroll
+                        for (int mm = 0; mm < 2; ++mm)
+#pragma unroll
+                            for (int nn = 0; nn < 4; ++nn)
+#pragma unroll
+                                for (int e = 0; e < 2; ++e) {
+                                    const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t + e;
+                                    if (cc <= r && 64 + r < nloc) S22[r * potf2::SLDP + cc] -= o[mm][nn][e];
+                                }
+                        cons_sync();
+                    }
+                }
+                potf2::gemm64(S21, W11, true, warp, lane, o);                      // Tm = L21 W11
+                cons_sync();
+#pragma unroll
+                for (int mm = 0; mm < 2; ++mm)
+#pragma unroll
+                    for (int nn = 0; nn < 4; ++nn) {
+                        const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t;
+                        S21[r * potf2::SLDP + cc] = o[mm][nn][0];
+                        S21[r * potf2::SLDP + cc + 1] = o[mm][nn][1];
+                    }
+                cons_sync();
+                potf2::gemm64(W22, S21, true, warp, lane, o);                      // W21 = -W22 Tm
+                double* Wg = a.Wbuf + ((size_t)c * T + j) * TB * TB;
+#pragma unroll
+                for (int mm = 0; mm < 2; ++mm)
+#pragma unroll
+                    for (int nn = 0; nn < 4; ++nn) {
+                        const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t;
+                        *reinterpret_cast<double2*>(Wg + (size_t)(64 + r) * TB + cc) = make_double2(-o[mm][nn][0], -o[mm][nn][1]);
+                    }
+                // L11, L22 -> the matrix (lower triangle only); W11, 0, W22 -> Wbuf
+                for (int idx = tid; idx < 64 * 64; idx += NCONS) {
+                    const int r = idx >> 6, cc = idx & 63;
+                    if (cc <= r) {
+                        if (tn0 + r < M) A[(size_t)(tn0 + r) * ld + tn0 + cc] = S11[r * potf2::SLDP + cc];
+                        if (tn0 + 64 + r < M) A[(size_t)(tn0 + 64 + r) * ld + tn0 + 64 + cc] = S22[r * potf2::SLDP + cc];
+                    }
+                    Wg[(size_t)r * TB + cc] = W11[r * potf2::SLDP + cc];
+                    Wg[(size_t)r * TB + 64 + cc] = 0.0;
+                    Wg[(size_t)(64 + r) * TB + 64 + cc] = W22[r * potf2::SLDP + cc];
+                }
+                __threadfence();
+                fence_proxy_async();
+                cons_sync();
+                if (tid == 0) {
+                    if (sFail != 0 && a.info != nullptr && a.info[c] == 0) a.info[c] = sFail;
+                    st_release_gpu(flags_c + (size_t)j * T + j, a.epoch);
+                }
+            }
+            git += (uint32_t)(KT + KE);
+            __syncthreads();
+            if (tid == 0) sTicket = atomicAdd(a.ticket, 1u) - a.ticket_base;
+            __syncthreads();
+        }
+    }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn()
+{
+    static EncodeTiledFn fn = nullptr;           // a driver entry point, not library state
+    if (fn == nullptr) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+}  // namespace
+
+size_t bdk_potrf_tiles_scratch_bytes(const bd_ctx* ctx)
+{
+    const size_t T = (size_t)(ctx->M + TB - 1) / TB;
+    return sizeof(double) * (size_t)ctx->C * T * TB * TB;
+}
+
+int bdk_potrf_tiles(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
+{
+    const int M = ctx->M, C = ctx->C, T = (M + TB - 1) / TB;
+    const uint64_t total64 = (uint64_t)C * T * (T + 1) / 2;
+    if (total64 + 1024 > 0xffffffffull || (uint64_t)C * T * TB > 0x7fffffffull) return BD_ERR_ALLOC;
+    if (ctx->tile_W == nullptr) {
+        BD_CUDA(ctx, cudaMalloc(&ctx->tile_W, bdk_potrf_tiles_scratch_bytes(ctx)));
+        const size_t fb = sizeof(int) * ((size_t)C * T * T + 2);
+        BD_CUDA(ctx, cudaMalloc(&ctx->tile_flags, fb));
+        BD_CUDA(ctx, cudaMemsetAsync(ctx->tile_flags, 0, fb, ctx->stream));
+        ctx->tile_epoch = 0;
+        ctx->tile_ticket_base = 0;
+        BD_CUDA(ctx, cudaFuncSetAttribute(k_potrf_tiles, cudaFuncAttributeMaxDynamicSharedMemorySize, TILE_SMEM));
+    }
+    EncodeTiledFn enc = encode_fn();
+    if (enc == nullptr) { ctx->last_cuda = cudaErrorNotSupported; return BD_ERR_CUDA; }
+    if (ctx->tile_mapA_ptr != A || ctx->tile_mapA_ld != ld || ctx->tile_mapA_stride != stride) {
+        static_assert(sizeof(CUtensorMap) == sizeof(ctx->tile_maps[0]), "tensor map storage");
+        CUtensorMap* mA = reinterpret_cast<CUtensorMap*>(&ctx->tile_maps[0]);
+        CUtensorMap* mW = reinterpret_cast<CUtensorMap*>(&ctx->tile_maps[1]);
+        // columns beyond M read as zero (the ragged last tile column), rows beyond M likewise
+        const cuuint64_t dimA[3] = {(cuuint64_t)M, (cuuint64_t)M, (cuuint64_t)C};
+        const cuuint64_t strA[2] = {(cuuint64_t)ld * 8, (cuuint64_t)stride * 8};
+        const cuuint32_t boxA[3] = {BOXK, TB, 1}, es3[3] = {1, 1, 1};
+        CUresult r1 = enc(mA, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, A, dimA, strA, boxA, es3, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        const cuuint64_t dimW[2] = {(cuuint64_t)TB, (cuuint64_t)C * T * TB};
+        const cuuint64_t strW[1] = {(cuuint64_t)TB * 8};
+        const cuuint32_t boxW[2] = {BOXK, TB}, es2[2] = {1, 1};
+        CUresult r2 = enc(mW, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, ctx->tile_W, dimW, strW, boxW, es2, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r1 != CUDA_SUCCESS || r2 != CUDA_SUCCESS) { ctx->last_cuda = cudaErrorInvalidValue; return BD_ERR_CUDA; }
+        ctx->tile_mapA_ptr = A; ctx->tile_mapA_ld = ld; ctx->tile_mapA_stride = stride;
+    }
+    TileArgs a;
+    a.A = A; a.ld = ld; a.stride = stride; a.M = M; a.C = C; a.T = T;
+    a.Wbuf = ctx->tile_W;
+    a.flags = ctx->tile_flags;
+    a.epoch = ++ctx->tile_epoch;
+    a.ticket = reinterpret_cast<unsigned*>(ctx->tile_flags + (size_t)C * T * T);
+    a.err = ctx->tile_flags + (size_t)C * T * T + 1;
+    a.ticket_base = ctx->tile_ticket_base;
+    a.total = (unsigned)total64;
+    a.info = info;
+    const unsigned grid = (a.total < (unsigned)ctx->num_sms) ? a.total : (unsigned)ctx->num_sms;
+    ctx->tile_ticket_base += a.total + grid;          // every CTA draws exactly one ticket beyond the last tile
+    BD_LAUNCH(ctx, k_potrf_tiles, dim3(grid), dim3(NTHREADS), TILE_SMEM, *reinterpret_cast<const CUtensorMap*>(&ctx->tile_maps[0]),
+              *reinterpret_cast<const CUtensorMap*>(&ctx->tile_maps[1]), a);
+    return 0;
+}
