@@ -7,7 +7,7 @@
 //                                                                    C tile never leaves the accumulators
 //     i > j:  S = -acc;  L_ij = S W_j^T  with W_j = L_jj^-1          a second, 128-deep pass through the same pipeline
 //     i = j:  L_jj = chol(S), W_j = L_jj^-1                          in shared memory (potf2_blocked.cuh, 64 + 64)
-//   Tickets are handed out column by column (j outer, then chain, then i); a tile waits (ld.acquire on the ready flag
+//   Tickets are handed out column by column (j outer, then chain, then i, the next diagonal tile early); a tile waits (ld.acquire on the ready flag
 //   of the tiles it reads) only for tiles with SMALLER tickets, which running CTAs own, so the schedule cannot
 //   deadlock and needs no co-residency.  Later columns start while the diagonal block of the current one is still being
 //   factored: the lookahead that the multi-launch version (potrf.cu) does not have, and one launch instead of
@@ -74,21 +74,29 @@ __device__ __forceinline__ void wait_flag(const int* f, int epoch, int* err)
     }
 }
 
-// ticket -> (column j, chain c, row i): columns in order, inside a column chain by chain, inside a chain i = j .. T-1
+// ticket -> (row i, column j, chain c).  Order: first the diagonal tile (0, 0) of every chain; then, for j = 0 .. T-2 and
+// inside it chain by chain, the tiles of column j with the NEXT diagonal tile slipped in early:
+//     (j+1, j), (j+1, j+1), (j+2, j), .., (T-1, j).
+// Tile (j+1, j+1) only needs row j+1 up to column j, so it can be factored while the rest of column j is still being
+// computed: when the tiles of column j+1 come up, L_{j+1,j+1} and its inverse have long been published.  Every tile
+// depends on tiles with smaller tickets only.
 __device__ __forceinline__ void decode_ticket(unsigned tk, int C, int T, int& j, int& c, int& i)
 {
-    const long long q = (long long)(tk / (unsigned)C);         // tiles of one chain in the columns before: j T - j (j-1) / 2 <= q
+    if (tk < (unsigned)C) { i = 0; j = 0; c = (int)tk; return; }
+    const unsigned u = tk - (unsigned)C;
+    const long long q = (long long)(u / (unsigned)C);          // entries of one chain in the phases before: j T - j (j-1) / 2 <= q
     const double b = 2.0 * T + 1.0;
     int jj = (int)((b - sqrt(fmax(b * b - 8.0 * (double)q, 0.0))) * 0.5);
-    jj = max(0, min(jj, T - 1));
+    jj = max(0, min(jj, T - 2));
     auto before = [&](int x) { return (long long)x * T - (long long)x * (x - 1) / 2; };
-    while (jj + 1 < T && before(jj + 1) * C <= (long long)tk) ++jj;
-    while (jj > 0 && before(jj) * C > (long long)tk) --jj;
-    const long long rem = (long long)tk - before(jj) * C;
-    const int w = T - jj;
-    j = jj;
+    while (jj + 1 <= T - 2 && before(jj + 1) * C <= (long long)u) ++jj;
+    while (jj > 0 && before(jj) * C > (long long)u) --jj;
+    const long long rem = (long long)u - before(jj) * C;
+    const int w = T - jj;                                       // entries per chain in phase jj
     c = (int)(rem / w);
-    i = jj + (int)(rem - (long long)c * w);
+    const int idx = (int)(rem - (long long)c * w);
+    if (idx == 1) { i = jj + 1; j = jj + 1; }
+    else { i = jj + (idx == 0 ? 1 : idx); j = jj; }
 }
 
 __global__ void __launch_bounds__(NTHREADS, 1) k_potrf_tiles(const __grid_constant__ CUtensorMap tmA,
