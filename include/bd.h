@@ -131,6 +131,13 @@ int bd_step(bd_ctx *ctx, double *r_dev, uint64_t first_step, int32_t n_steps);
  * Either output may be NULL.                                                                     */
 int bd_observables(bd_ctx *ctx, const double *r_dev, double *per_chain_dev, double *ensemble_dev);
 
+/* Relaxation-time observable ("the time scale of the decay of the autocorrelation function of the
+ * end-to-end vector", fitted over its last 70 %).  bd_end_to_end writes R_dev [C][3] = r_N - r_0 (the origin R(0) of a
+ * run); bd_autocorr writes out_dev[3] = { sum_c R.R0, sum_c (R.R0)^2, sum_c R0.R0 } for the current positions, so that
+ * C(t) = out[0] / out[2] and its standard error follow on the host (reading B3: ensemble average at lag t).  */
+int bd_end_to_end(bd_ctx *ctx, const double *r_dev, double *R_dev);
+int bd_autocorr(bd_ctx *ctx, const double *r_dev, const double *R0_dev, double *out_dev);
+
 /* Synchronises the stream; number of chains whose info != 0 since the last call that reset it
  * (bd_step / bd_cholesky with info_dev == NULL reset at entry), and the first such chain (-1).   */
 int bd_last_info(bd_ctx *ctx, int32_t *n_failed_chains, int32_t *first_failed_chain);

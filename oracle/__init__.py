@@ -261,5 +261,21 @@ def observables(p: Params, r):
     return per, ens
 
 
+def end_to_end(n_rods: int, r) -> np.ndarray:
+    """r[C][N_b][3] -> R[C][3] = r_N - r_0."""
+    r = _f64(r)
+    R = np.empty((r.shape[0], 3), dtype=np.float64)
+    lib().orc_end_to_end(C.c_int32(n_rods), C.c_int32(r.shape[0]), _ptr(r), _ptr(R))
+    return R
+
+
+def autocorr(n_rods: int, r, R0) -> np.ndarray:
+    """(sum_c R.R0, sum_c (R.R0)^2, sum_c R0.R0) of the end-to-end vectors."""
+    r, R0 = _f64(r), _f64(R0)
+    out = np.empty(3, dtype=np.float64)
+    lib().orc_autocorr(C.c_int32(n_rods), C.c_int32(r.shape[0]), _ptr(r), _ptr(R0), _ptr(out))
+    return out
+
+
 def num_threads() -> int:
     return int(lib().orc_num_threads())

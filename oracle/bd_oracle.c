@@ -452,6 +452,38 @@ void orc_observables(const orc_params *p, int32_t C, const double *r, double *pe
         }
 }
 
+/* ---------------------------------------------------------------------------------------
+ * End-to-end vector and its autocorrelation (the relaxation time is "the time scale of
+ * the decay of the autocorrelation function of the end-to-end vector of the chain", fitted over its
+ * last 70 %; reading B3: ensemble average at lag t from a common origin,
+ * C(t) = <R(t).R(0)> / <R(0).R(0)>).
+ *   R_c = r_N - r_0                                          (Eq. 25's vector)
+ *   out[0] = sum_c R_c.R0_c, out[1] = sum_c (R_c.R0_c)^2, out[2] = sum_c R0_c.R0_c
+ * ------------------------------------------------------------------------------------- */
+void orc_end_to_end(int32_t n_rods, int32_t C, const double *r, double *R)
+{
+    size_t M = 3 * ((size_t)n_rods + 1);
+    for (int32_t c = 0; c < C; ++c)
+        for (int d = 0; d < 3; ++d) R[3 * (size_t)c + d] = r[c * M + 3 * (size_t)n_rods + d] - r[c * M + d];
+}
+
+void orc_autocorr(int32_t n_rods, int32_t C, const double *r, const double *R0, double out[3])
+{
+    size_t M = 3 * ((size_t)n_rods + 1);
+    out[0] = out[1] = out[2] = 0.0;
+    for (int32_t c = 0; c < C; ++c) {
+        double dot = 0.0, n0 = 0.0;
+        for (int d = 0; d < 3; ++d) {
+            double Rd = r[c * M + 3 * (size_t)n_rods + d] - r[c * M + d];
+            dot += Rd * R0[3 * (size_t)c + d];
+            n0 += R0[3 * (size_t)c + d] * R0[3 * (size_t)c + d];
+        }
+        out[0] += dot;
+        out[1] += dot * dot;
+        out[2] += n0;
+    }
+}
+
 int32_t orc_num_threads(void)
 {
 #ifdef _OPENMP

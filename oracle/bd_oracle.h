@@ -103,6 +103,11 @@ void   orc_observables_chain(const orc_params *p, const double *r, double obs[OR
 void   orc_observables(const orc_params *p, int32_t C, const double *r,
                        double *per_chain /* [C][ORC_NOBS] */, double *ensemble /* [2][ORC_NOBS] */);
 
+/* end-to-end vectors R[C][3] = r_N - r_0 and their autocorrelation sums against R0:
+ * out = { sum_c R.R0, sum_c (R.R0)^2, sum_c R0.R0 }                                           */
+void   orc_end_to_end(int32_t n_rods, int32_t C, const double *r, double *R);
+void   orc_autocorr(int32_t n_rods, int32_t C, const double *r, const double *R0, double out[3]);
+
 int32_t orc_num_threads(void);
 
 #ifdef __cplusplus

@@ -28,7 +28,7 @@ class bd_params(C.Structure):
 
 EXPORTS = ("bd_create", "bd_destroy", "bd_workspace_bytes", "bd_set_workspace", "bd_set_flow",
            "bd_init_random_walk", "bd_assemble_hi", "bd_cholesky", "bd_brownian", "bd_noise", "bd_drift",
-           "bd_update", "bd_set_path", "bd_set_cholesky", "bd_step", "bd_observables", "bd_last_info", "bd_step_host", "bd_profile",
+           "bd_update", "bd_set_path", "bd_set_cholesky", "bd_step", "bd_observables", "bd_end_to_end", "bd_autocorr", "bd_last_info", "bd_step_host", "bd_profile",
            "bd_stage_ms", "bd_launch_count", "bd_strerror", "bd_last_error")
 
 _lib = None
@@ -61,6 +61,8 @@ def load_library(path: str | None = None) -> C.CDLL:
     lib.bd_set_cholesky.argtypes = [vp, i32]
     lib.bd_step.argtypes = [vp, dp, u64, i32]
     lib.bd_observables.argtypes = [vp, dp, dp, dp]
+    lib.bd_end_to_end.argtypes = [vp, dp, dp]
+    lib.bd_autocorr.argtypes = [vp, dp, dp, dp]
     lib.bd_last_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i32)]
     lib.bd_step_host.argtypes = [vp, dp, u64, i32, dp]
     lib.bd_profile.argtypes = [vp, i32]
@@ -218,6 +220,17 @@ class BD:
         per, ens = self.empty(self.C, NOBS), self.empty(2, NOBS)
         self._check("bd_observables", self.lib.bd_observables(self._ctx, _dptr(r), _dptr(per), _dptr(ens)))
         return per, ens
+
+    def end_to_end(self, r, R=None):
+        R = self.empty(self.C, 3) if R is None else R
+        self._check("bd_end_to_end", self.lib.bd_end_to_end(self._ctx, _dptr(r), _dptr(R)))
+        return R
+
+    def autocorr(self, r, R0, out=None):
+        """device tensor [3]: sum_c R.R0, sum_c (R.R0)^2, sum_c R0.R0."""
+        out = self.empty(3) if out is None else out
+        self._check("bd_autocorr", self.lib.bd_autocorr(self._ctx, _dptr(r), _dptr(R0), _dptr(out)))
+        return out
 
     def last_info(self):
         n, first = C.c_int32(0), C.c_int32(-1)

@@ -293,6 +293,23 @@ int bd_observables(bd_ctx* ctx, const double* r_dev, double* per_chain_dev, doub
     return bdk_observables(ctx, r_dev, per_chain_dev, ensemble_dev);
 }
 
+int bd_end_to_end(bd_ctx* ctx, const double* r_dev, double* R_dev)
+{
+    if (ctx == nullptr) return -1;
+    if (r_dev == nullptr) return -2;
+    if (R_dev == nullptr) return -3;
+    return bdk_end_to_end(ctx, r_dev, R_dev);
+}
+
+int bd_autocorr(bd_ctx* ctx, const double* r_dev, const double* R0_dev, double* out_dev)
+{
+    if (ctx == nullptr) return -1;
+    if (r_dev == nullptr) return -2;
+    if (R0_dev == nullptr) return -3;
+    if (out_dev == nullptr) return -4;
+    return bdk_autocorr(ctx, r_dev, R0_dev, out_dev);
+}
+
 int bd_last_info(bd_ctx* ctx, int32_t* n_failed_chains, int32_t* first_failed_chain)
 {
     if (ctx == nullptr) return -1;

@@ -82,6 +82,8 @@ int bdk_drift(bd_ctx* ctx, const double* r, double* T, double* F, double* v);
 int bdk_update(bd_ctx* ctx, const double* r, const double* v, const double* y, const int32_t* info_step,
                int32_t* info_sticky, double* r_out);
 int bdk_observables(bd_ctx* ctx, const double* r, double* per_chain, double* ensemble);
+int bdk_end_to_end(bd_ctx* ctx, const double* r, double* R);
+int bdk_autocorr(bd_ctx* ctx, const double* r, const double* R0, double* out);
 int bdk_count_failures(bd_ctx* ctx, const int32_t* info);
 bool bdk_chain_step_supported(const bd_ctx* ctx);
 int bdk_chain_step(bd_ctx* ctx, double* r, uint64_t first_step, int n_steps);

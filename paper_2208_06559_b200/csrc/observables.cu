@@ -105,7 +105,60 @@ __global__ void __launch_bounds__(256) k_count_failures(int C, const int32_t* __
     if (threadIdx.x == 0) { fail[0] = s_cnt; fail[1] = (s_first == 0x7fffffff) ? -1 : s_first; }
 }
 
+// End-to-end vectors R_c = r_N - r_0 (Eq. 25's vector), one thread per chain.
+__global__ void __launch_bounds__(256) k_end_to_end(int N, int C, const double* __restrict__ r_all, double* __restrict__ R_all)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= C) return;
+    const double* r = r_all + (size_t)c * 3 * (N + 1);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) R_all[3 * (size_t)c + d] = r[3 * N + d] - r[d];
+}
+
+// Autocorrelation sums of the end-to-end vector against a stored origin R0 (the relaxation time is the
+// decay time of this function): out = { sum_c R.R0, sum_c (R.R0)^2, sum_c R0.R0 }.  ONE CTA, fixed summation order
+// (deterministic, no atomics): the sums are 3 doubles per sampling instant.
+__global__ void __launch_bounds__(256) k_autocorr(int N, int C, const double* __restrict__ r_all, const double* __restrict__ R0_all,
+                                                  double* __restrict__ out)
+{
+    __shared__ double s_red[8][3];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+    for (int c = threadIdx.x; c < C; c += blockDim.x) {
+        const double* r = r_all + (size_t)c * 3 * (N + 1);
+        const double* R0 = R0_all + 3 * (size_t)c;
+        double dot = 0.0, n0 = 0.0;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const double Rd = r[3 * N + d] - r[d];
+            dot += Rd * R0[d];
+            n0 += R0[d] * R0[d];
+        }
+        a0 += dot; a1 += dot * dot; a2 += n0;
+    }
+    a0 = warp_sum(a0); a1 = warp_sum(a1); a2 = warp_sum(a2);
+    if (lane == 0) { s_red[warp][0] = a0; s_red[warp][1] = a1; s_red[warp][2] = a2; }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t += s_red[w][threadIdx.x];
+        out[threadIdx.x] = t;
+    }
+}
+
 }  // namespace
+
+int bdk_end_to_end(bd_ctx* ctx, const double* r, double* R)
+{
+    BD_LAUNCH(ctx, k_end_to_end, dim3((ctx->C + 255) / 256), dim3(256), 0, ctx->N, ctx->C, r, R);
+    return 0;
+}
+
+int bdk_autocorr(bd_ctx* ctx, const double* r, const double* R0, double* out)
+{
+    BD_LAUNCH(ctx, k_autocorr, dim3(1), dim3(256), 0, ctx->N, ctx->C, r, R0, out);
+    return 0;
+}
 
 int bdk_observables(bd_ctx* ctx, const double* r, double* per_chain, double* ensemble)
 {

@@ -7,7 +7,8 @@ dt = 0.001, K* = 1000, expected scaling R_ee, R_g ~ N^0.5 and lambda ~ N^1.5 wit
 Instead of one chain for 100 relaxation times (the paper's single-chain-per-GPU protocol) an ENSEMBLE of independent
 chains is followed for `--window` Rouse times from equilibrium random-walk starts and the normalised correlation
 C(t) = <R(t).R(0)> / <R(0).R(0)> is averaged over the chains.  All time stepping is `bd_step` (many steps per launch);
-torch is used only to read the end-to-end vectors between launches and for the least-squares fit.  This replaces the
+the correlation sums come from `bd_end_to_end` / `bd_autocorr` (kernels of libbd, oracle counterpart orc_autocorr); numpy
+is used for the least-squares fit on the host only.  This replaces the
 Rouse stand-in lambda_s of workloads.py (reading A12) by measured values.
 """
 from __future__ import annotations
@@ -29,16 +30,18 @@ def measure(n_rods: int, n_chains: int, hstar: float, dt: float, window: float, 
     bd = BD(n_rods=n_rods, n_chains=n_chains, dt=dt, hstar=hstar, seed=seed)       # K* = 1/dt, a = h* b (or a = b/2 if h* = 0)
     bd.set_workspace()
     r = bd.init_random_walk(4242)
-    R0 = (r[:, -1, :] - r[:, 0, :]).clone()
-    norm = float((R0 * R0).sum(dim=1).mean())
-    t, acf = [0.0], [1.0]
+    R0 = bd.end_to_end(r)                                   # origin R(0) of every chain, kept on the device
+    sums = bd.empty(samples + 1, 3)                         # per sampling instant: sum R.R0, sum (R.R0)^2, sum R0.R0
+    bd.autocorr(r, R0, sums[0])
+    t = [0.0]
     step = 0
-    for _ in range(samples):
+    for k in range(samples):
         bd.step(r, first_step=step, n_steps=stride)
         step += stride
-        R = r[:, -1, :] - r[:, 0, :]
+        bd.autocorr(r, R0, sums[k + 1])                     # k_autocorr in libbd (no torch arithmetic on the path)
         t.append(step * dt)
-        acf.append(float((R * R0).sum(dim=1).mean()) / norm)
+    sums_h = sums.cpu().numpy()                             # one read-back at the end
+    acf = list(sums_h[:, 0] / sums_h[0, 2])
     per, _ = bd.observables(r)
     torch.cuda.synchronize()
     assert bd.last_info() == (0, -1)

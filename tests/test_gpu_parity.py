@@ -396,3 +396,27 @@ def test_bad_arguments_are_rejected_without_launching():
         bd.assemble_hi(torch.zeros(1, 6, 3, dtype=torch.float64, device="cuda"),
                        torch.zeros(1, 18, 17, dtype=torch.float64, device="cuda"))      # ld odd and < M
     assert e.value.code == -4 and bd.launch_count() == n0
+
+
+# ------------------------------------------------------------------------------------------ f1: relaxation-time observable
+@pytest.mark.parametrize("N,C", [(1, 3), (20, 300), (100, 1000)])
+def test_end_to_end_and_autocorrelation_match_oracle(N, C):
+    """bd_end_to_end / bd_autocorr against orc_end_to_end / orc_autocorr on moved chains."""
+    r0 = W.random_chains(C, N, seed=900 + N, rod_jitter=0.01)
+    r1 = W.random_chains(C, N, seed=901 + N, rod_jitter=0.01) * 0.3 + r0           # correlated with r0, not equal
+    bd = _bd(N, C)
+    R0 = bd.end_to_end(_dev(r0))
+    assert np.array_equal(_host(R0), O.end_to_end(N, r0))
+    out = _host(bd.autocorr(_dev(r1), R0))
+    want = O.autocorr(N, r1, O.end_to_end(N, r0))
+    assert np.allclose(out, want, rtol=1e-12, atol=0)
+    assert np.allclose(_host(bd.autocorr(_dev(r0), R0)), O.autocorr(N, r0, O.end_to_end(N, r0)), rtol=1e-12)
+
+
+def test_relaxation_time_pipeline_free_draining():
+    """relaxation.measure on the GPU path (bd_step + bd_autocorr): without HI a 10-rod chain relaxes on the Rouse
+    scale (the paper's Fig. 8 check); round 1 measured lambda = 1.27 lambda_Rouse for bead-rod chains."""
+    from paper_2208_06559_b200 import relaxation
+    row = relaxation.measure(10, 2048, 0.0, 1e-3, 2.0, 50)
+    assert 0.9 < row["lambda"] / row["lambda_rouse"] < 1.7
+    assert abs(row["Ree"] ** 2 / 10.0 - 1.0) < 0.1                                # <R^2> = N b^2 at equilibrium

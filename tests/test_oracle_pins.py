@@ -532,6 +532,35 @@ def test_initial_walk_follows_the_purpose_one_counter_layout():
         O.philox4x32_10([0, chain, 0, 1 << 28], [seed & 0xFFFFFFFF, seed >> 32])
 
 
+def test_end_to_end_autocorrelation_closed_forms():
+    """PAPER.md:283 (relaxation time from the autocorrelation of the end-to-end vector; reading B3: ensemble at lag t).
+    (i) two chains written out by hand; (ii) every chain rigidly rotated by theta about its own axis perpendicular
+    to R0: sum R.R0 = cos(theta) sum |R0|^2; (iii) translation of the chains changes nothing; (iv) t = 0 gives 1."""
+    N = 2
+    r = np.array([[[0, 0, 0], [1, 0, 0], [1, 2, 2]], [[1, 1, 1], [0, 0, 0], [-1, 1, 4]]], dtype=float)
+    R = O.end_to_end(N, r)
+    assert np.array_equal(R, [[1, 2, 2], [-2, 0, 3]])
+    R0 = np.array([[2, -1, 0.5], [1, 1, 1]])
+    out = O.autocorr(N, r, R0)
+    # chain 0: (1,2,2).(2,-1,0.5) = 1; chain 1: (-2,0,3).(1,1,1) = 1;  |R0|^2 = 5.25 and 3
+    assert out == pytest.approx([2.0, 2.0, 8.25], rel=1e-15)
+    rng = np.random.default_rng(11)
+    C, N = 50, 7
+    r = W.random_chains(C, N, seed=4)
+    R0 = O.end_to_end(N, r)
+    assert O.autocorr(N, r, R0) == pytest.approx([(R0 ** 2).sum(), ((R0 ** 2).sum(1) ** 2).sum(), (R0 ** 2).sum()], rel=1e-14)
+    theta = 0.7
+    rot = np.empty_like(r)
+    for c in range(C):
+        axis = np.cross(R0[c], rng.standard_normal(3)); axis /= np.linalg.norm(axis)       # perpendicular to R0
+        K = np.array([[0, -axis[2], axis[1]], [axis[2], 0, -axis[0]], [-axis[1], axis[0], 0]])
+        Rm = np.eye(3) + math.sin(theta) * K + (1 - math.cos(theta)) * K @ K                # Rodrigues
+        rot[c] = r[c] @ Rm.T + rng.standard_normal(3)                                       # rotated and shifted
+    out = O.autocorr(N, rot, R0)
+    assert out[0] == pytest.approx(math.cos(theta) * (R0 ** 2).sum(), rel=1e-12)
+    assert out[2] == pytest.approx((R0 ** 2).sum(), rel=1e-14)
+
+
 def test_failure_leaves_state_unchanged():
     """A10: coincident beads with h* = a make D singular -> reported, state untouched."""
     r = np.array([[0, 0, 0], [1.0, 0, 0], [0, 0, 0]], dtype=float)     # bead 2 on top of bead 0
