@@ -20,6 +20,8 @@
 //   SYRK/GEMM symmetry: A and B fragments index the k dimension identically, so a lane may read ANY k of the slab as
 //   long as both operands use the same map: lane (g, t) reads 16-byte chunk (2 t + j) ^ g of row g (j = 0, 1), which
 //   is conflict free under the 128-byte swizzle (the 8 lanes of a quarter-warp hit 8 distinct chunks).
+#include <type_traits>
+
 #include <cuda.h>          // CUtensorMap and its enums only; cuTensorMapEncodeTiled is fetched through the runtime (no -lcuda)
 
 #include "bd_internal.cuh"
@@ -33,6 +35,7 @@ constexpr int BOXK = 16;                      // columns per TMA box (128 bytes 
 constexpr int BK = 32;                        // columns per ring stage (two boxes per operand)
 constexpr int SPB = TB / BK;                  // stages per 128-column block
 constexpr int STAGES = 3;
+constexpr int QD = 2;                         // depth of the ticket queue between the producer and the consumers
 constexpr int BOX_BYTES = TB * BOXK * 8;      // 16 KB
 constexpr int STAGE_BYTES = 4 * BOX_BYTES;    // A box 0, A box 1, B box 0, B box 1
 constexpr int NCONS = 256;                    // consumer threads (8 warps)
@@ -99,12 +102,51 @@ __device__ __forceinline__ void decode_ticket(unsigned tk, int C, int T, int& j,
     else { i = jj + (idx == 0 ? 1 : idx); j = jj; }
 }
 
+// One 128 x 16 box of both operands: 2 chunk pairs x (4 + (8 - NTLO) LDS.128, 2 x 4 x (8 - NTLO) DMMA) per warp.  NTLO > 0 skips
+// the first n-tiles (the S W^T pass: W is lower triangular, column block nt of the warp needs p <= its last column only).
+template <int NTLO>
+__device__ __forceinline__ void compute_box(double (&acc)[4][8][2], const uint8_t* __restrict__ sa, const uint8_t* __restrict__ sb,
+                                            const int xo0, const int xo1)
+{
+#pragma unroll
+    for (int jj = 0; jj < 2; ++jj) {
+        const int xo = jj ? xo1 : xo0;
+        double2 af[4], bf[8];
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt) af[mt] = *reinterpret_cast<const double2*>(sa + mt * 1024 + xo);
+#pragma unroll
+        for (int nt = NTLO; nt < 8; ++nt) bf[nt] = *reinterpret_cast<const double2*>(sb + nt * 1024 + xo);
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+            for (int nt = NTLO; nt < 8; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], af[mt].x, bf[nt].x);
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+            for (int nt = NTLO; nt < 8; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], af[mt].y, bf[nt].y);
+    }
+}
+
+// box B8 (16 columns p = 16 B8 ..) of the S W^T pass for the warp column half wn: X[., cc] needs p <= cc
+template <int B8>
+__device__ __forceinline__ void trsm_box(double (&acc)[4][8][2], const int wn, const uint8_t* sa, const uint8_t* sb, const int xo0,
+                                         const int xo1)
+{
+    if (wn == 0) {
+        if constexpr (B8 < 4) compute_box<2 * B8>(acc, sa, sb, xo0, xo1);        // columns 0..63: p < 64 only
+    } else {
+        if constexpr (B8 < 4) compute_box<0>(acc, sa, sb, xo0, xo1);
+        else compute_box<2 * (B8 - 4)>(acc, sa, sb, xo0, xo1);
+    }
+}
+
 __global__ void __launch_bounds__(NTHREADS, 1) k_potrf_tiles(const __grid_constant__ CUtensorMap tmA,
                                                              const __grid_constant__ CUtensorMap tmW, const TileArgs a)
 {
     extern __shared__ uint8_t smem_raw[];
-    __shared__ __align__(8) uint64_t sBar[2 * STAGES + 1];     // full[0..S), empty[S..2S), S-stored
-    __shared__ unsigned sTicket;
+    // full[0..S), empty[S..2S), S-stored, diagonal-tile-done, ticket queue full[QD], ticket queue empty[QD]
+    __shared__ __align__(8) uint64_t sBar[2 * STAGES + 2 + 2 * QD];
+    __shared__ unsigned sQ[QD];
     __shared__ int sFail;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -112,318 +154,316 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_potrf_tiles(const __grid_consta
     const int g = lane >> 2, t = lane & 3;
     const uint32_t ring = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* ring_g = smem_raw + (ring - smem_u32(smem_raw));
-    const uint32_t bar_full = smem_u32(&sBar[0]), bar_empty = smem_u32(&sBar[STAGES]), bar_s = smem_u32(&sBar[2 * STAGES]);
+    const uint32_t bar_full = smem_u32(&sBar[0]), bar_empty = smem_u32(&sBar[STAGES]), bar_s = smem_u32(&sBar[2 * STAGES]),
+                   bar_d = smem_u32(&sBar[2 * STAGES + 1]), bar_qf = smem_u32(&sBar[2 * STAGES + 2]),
+                   bar_qe = smem_u32(&sBar[2 * STAGES + 2 + QD]);
 
     if (tid == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, NCONS / 32); }
         mbar_init(bar_s, NCONS);
+        mbar_init(bar_d, NCONS / 32);
+        for (int s = 0; s < QD; ++s) { mbar_init(bar_qf + 8 * s, 1); mbar_init(bar_qe + 8 * s, NCONS / 32); }
         mbar_fence_init();
-        sTicket = atomicAdd(a.ticket, 1u) - a.ticket_base;
     }
     __syncthreads();
 
-    uint32_t git = 0;          // ring stages consumed so far (same value in every thread)
-    uint32_t sphase = 0;       // uses of the S-stored barrier so far
     const int M = a.M, T = a.T;
     const int64_t ld = a.ld;
-    // fragment addressing inside a 128 x 16 box: row r at r * 128 bytes, logical 16-byte chunk q at (q ^ (r & 7)) * 16
-    const int xo0 = ((2 * t) ^ g) * 16, xo1 = ((2 * t + 1) ^ g) * 16;
-    const int offA = (wm * 32 + g) * 128, offB = (wn * 64 + g) * 128;
 
     // Register budget: 384 threads cap the kernel at 168 registers per thread (each of the 4 sub-partitions holds 3
     // warps); the producer warpgroup hands its share to the 8 consumer warps (64 accumulators + fragments) with
     // setmaxnreg.  The two roles run SEPARATE tile loops from here to the end of the kernel (ptxas allocates registers per
-    // region; after a common merge point it would have to assume the smaller budget) and meet at the two CTA barriers
-    // that end every tile.
+    // region) and talk through mbarriers only: the producer draws the tickets, publishes them in a 2-deep queue and runs
+    // AHEAD of the consumers (the next tile's first stages are in flight while the current tile is still in its epilogue);
+    // it only stops behind a diagonal tile, whose factorisation uses the ring as scratch.
     if (warp >= NCONS / 32) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(REGS_PRODUCER));
-        while (true) {
-            const unsigned tk = sTicket;
+        if (warp != NCONS / 32 || lane != 0) return;
+        // ================================== producer: one thread feeds the ring ==================================
+        uint32_t git = 0, sphase = 0, dphase = 0;      // ring stages issued, uses of the S-stored / diagonal-done barriers
+        for (uint32_t n = 0;; ++n) {
+            const unsigned tk = atomicAdd(a.ticket, 1u) - a.ticket_base;
+            const uint32_t qs = n % QD;
+            if (n >= QD) mbar_wait(bar_qe + 8 * qs, ((n / QD) - 1) & 1);
+            sQ[qs] = tk;
+            mbar_arrive(bar_qf + 8 * qs);              // release: the consumers read sQ after their wait
             if (tk >= a.total) break;
             int i, j, c;
             decode_ticket(tk, a.C, T, j, c, i);
             const bool diag = (i == j);
-            const int KT = j * SPB;                       // ring stages of the K loop
-            const int KE = diag ? 0 : SPB;                // ring stages of the S W^T pass
+            const int KT = j * SPB;                    // ring stages of the K loop
             int* flags_c = a.flags + (size_t)c * T * T;
             const int tm0 = i * TB, tn0 = j * TB;
-            // ============================== producer: one thread feeds the ring ==============================
-            if (warp == NCONS / 32 && lane == 0) {
-                auto acquire_slot = [&](uint32_t G) {
-                    const uint32_t sl = G % STAGES;
-                    if (G >= STAGES) mbar_wait(bar_empty + 8 * sl, ((G / STAGES) - 1) & 1);
-                    return sl;
-                };
-                int ready = 0;                        // 128-column blocks known to be final in rows i and j
-                if (j > 0 && ld_acquire_gpu(flags_c + (size_t)i * T + j - 1) == a.epoch &&
-                    ld_acquire_gpu(flags_c + (size_t)j * T + j - 1) == a.epoch) {
-                    ready = j;                        // tile (., j-1) final => every (., k < j-1) it read is final too
-                    fence_proxy_async();
+            auto acquire_slot = [&](uint32_t G) {
+                const uint32_t sl = G % STAGES;
+                if (G >= STAGES) mbar_wait(bar_empty + 8 * sl, ((G / STAGES) - 1) & 1);
+                return sl;
+            };
+            int ready = 0;                             // 128-column blocks known to be final in rows i and j
+            if (j > 0 && ld_acquire_gpu(flags_c + (size_t)i * T + j - 1) == a.epoch &&
+                ld_acquire_gpu(flags_c + (size_t)j * T + j - 1) == a.epoch) {
+                ready = j;                             // tile (., j-1) final => every (., k < j-1) it read is final too
+                fence_proxy_async();
+            }
+            for (int kb = 0; kb < j; ++kb) {
+                if (kb >= ready) {
+                    wait_flag(flags_c + (size_t)i * T + kb, a.epoch, a.err);
+                    if (!diag) wait_flag(flags_c + (size_t)j * T + kb, a.epoch, a.err);
+                    fence_proxy_async();               // the acquired tiles are read through the async proxy (TMA)
                 }
-                for (int kb = 0; kb < j; ++kb) {
-                    if (kb >= ready) {
-                        wait_flag(flags_c + (size_t)i * T + kb, a.epoch, a.err);
-                        if (!diag) wait_flag(flags_c + (size_t)j * T + kb, a.epoch, a.err);
-                        fence_proxy_async();          // the acquired tiles are read through the async proxy (TMA)
-                    }
-                    for (int s4 = 0; s4 < SPB; ++s4) {
-                        const uint32_t G = git + kb * SPB + s4, sl = acquire_slot(G);
-                        const uint32_t dst = ring + sl * STAGE_BYTES, fb = bar_full + 8 * sl;
-                        const int k0 = kb * TB + s4 * BK;
-                        mbar_expect_tx(fb, diag ? 2 * BOX_BYTES : 4 * BOX_BYTES);
-                        tma_tile_3d(dst, &tmA, k0, tm0, c, fb);
-                        tma_tile_3d(dst + BOX_BYTES, &tmA, k0 + BOXK, tm0, c, fb);
-                        if (!diag) {
-                            tma_tile_3d(dst + 2 * BOX_BYTES, &tmA, k0, tn0, c, fb);
-                            tma_tile_3d(dst + 3 * BOX_BYTES, &tmA, k0 + BOXK, tn0, c, fb);
-                        }
-                    }
-                }
-                if (!diag) {
-                    mbar_wait(bar_s, sphase & 1);     // the consumers have stored S (generic proxy) ...
-                    fence_proxy_async();              // ... which is now read back through TMA
-                    wait_flag(flags_c + (size_t)j * T + j, a.epoch, a.err);     // L_jj and W_j are final
-                    fence_proxy_async();
-                    for (int s4 = 0; s4 < SPB; ++s4) {
-                        const uint32_t G = git + KT + s4, sl = acquire_slot(G);
-                        const uint32_t dst = ring + sl * STAGE_BYTES, fb = bar_full + 8 * sl;
-                        mbar_expect_tx(fb, 4 * BOX_BYTES);
-                        tma_tile_3d(dst, &tmA, tn0 + s4 * BK, tm0, c, fb);                          // S[rows i][p]
-                        tma_tile_3d(dst + BOX_BYTES, &tmA, tn0 + s4 * BK + BOXK, tm0, c, fb);
-                        tma_tile_2d(dst + 2 * BOX_BYTES, &tmW, s4 * BK, (c * T + j) * TB, fb);      // W_j[cc][p]
-                        tma_tile_2d(dst + 3 * BOX_BYTES, &tmW, s4 * BK + BOXK, (c * T + j) * TB, fb);
+                for (int s4 = 0; s4 < SPB; ++s4) {
+                    const uint32_t G = git + kb * SPB + s4, sl = acquire_slot(G);
+                    const uint32_t dst = ring + sl * STAGE_BYTES, fb = bar_full + 8 * sl;
+                    const int k0 = kb * TB + s4 * BK;
+                    mbar_expect_tx(fb, diag ? 2 * BOX_BYTES : 4 * BOX_BYTES);
+                    tma_tile_3d(dst, &tmA, k0, tm0, c, fb);
+                    tma_tile_3d(dst + BOX_BYTES, &tmA, k0 + BOXK, tm0, c, fb);
+                    if (!diag) {
+                        tma_tile_3d(dst + 2 * BOX_BYTES, &tmA, k0, tn0, c, fb);
+                        tma_tile_3d(dst + 3 * BOX_BYTES, &tmA, k0 + BOXK, tn0, c, fb);
                     }
                 }
             }
-            __syncwarp();                             // lanes 1..31 wait here for the producer lane
-            git += (uint32_t)(KT + KE);
-            if (!diag) sphase += 1;
-            __syncthreads();                          // tile finished (the consumers may have used the ring as scratch)
-            __syncthreads();                          // next ticket published
+            git += (uint32_t)KT;
+            if (!diag) {
+                mbar_wait(bar_s, sphase & 1);          // the consumers have stored S (generic proxy) ...
+                ++sphase;
+                fence_proxy_async();                   // ... which is now read back through TMA
+                wait_flag(flags_c + (size_t)j * T + j, a.epoch, a.err);     // L_jj and W_j are final
+                fence_proxy_async();
+                for (int s4 = 0; s4 < SPB; ++s4) {
+                    const uint32_t G = git + s4, sl = acquire_slot(G);
+                    const uint32_t dst = ring + sl * STAGE_BYTES, fb = bar_full + 8 * sl;
+                    mbar_expect_tx(fb, 4 * BOX_BYTES);
+                    tma_tile_3d(dst, &tmA, tn0 + s4 * BK, tm0, c, fb);                          // S[rows i][p]
+                    tma_tile_3d(dst + BOX_BYTES, &tmA, tn0 + s4 * BK + BOXK, tm0, c, fb);
+                    tma_tile_2d(dst + 2 * BOX_BYTES, &tmW, s4 * BK, (c * T + j) * TB, fb);      // W_j[cc][p]
+                    tma_tile_2d(dst + 3 * BOX_BYTES, &tmW, s4 * BK + BOXK, (c * T + j) * TB, fb);
+                }
+                git += SPB;
+            } else {
+                mbar_wait(bar_d, dphase & 1);          // the ring is scratch until the diagonal tile is finished
+                ++dphase;
+            }
         }
-    } else {
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(REGS_CONSUMER));
-        while (true) {
-            const unsigned tk = sTicket;
-            if (tk >= a.total) break;
-            int i, j, c;
-            decode_ticket(tk, a.C, T, j, c, i);
-            const bool diag = (i == j);
-            const int KT = j * SPB;
-            const int KE = diag ? 0 : SPB;
-            double* A = a.A + (size_t)c * a.stride;
-            int* flags_c = a.flags + (size_t)c * T * T;
-            const int tm0 = i * TB, tn0 = j * TB;
-            // ============================== consumers: 8 warps, warp tile 32 x 64 =============================
-            // this warp's 32 x 64 block lies entirely above the diagonal of a diagonal tile -> no arithmetic
-            const bool warp_active = !diag || (wn * 64 <= wm * 32 + 31);
-            double acc[4][8][2];
+        return;
+    }
+
+    // ====================================== consumers: 8 warps, warp tile 32 x 64 ======================================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(REGS_CONSUMER));
+    // fragment addressing inside a 128 x 16 box: row r at r * 128 bytes, logical 16-byte chunk q at (q ^ (r & 7)) * 16
+    const int xo0 = ((2 * t) ^ g) * 16, xo1 = ((2 * t + 1) ^ g) * 16;
+    const int offA = (wm * 32 + g) * 128, offB = (wn * 64 + g) * 128;
+    uint32_t git = 0;                                  // ring stages consumed so far
+    for (uint32_t n = 0;; ++n) {
+        const uint32_t qs = n % QD;
+        mbar_wait(bar_qf + 8 * qs, (n / QD) & 1);
+        const unsigned tk = sQ[qs];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_qe + 8 * qs);
+        if (tk >= a.total) break;
+        int i, j, c;
+        decode_ticket(tk, a.C, T, j, c, i);
+        const bool diag = (i == j);
+        const int KT = j * SPB;
+        double* A = a.A + (size_t)c * a.stride;
+        int* flags_c = a.flags + (size_t)c * T * T;
+        const int tm0 = i * TB, tn0 = j * TB;
+        // this warp's 32 x 64 block lies entirely above the diagonal of a diagonal tile -> no arithmetic
+        const bool warp_active = !diag || (wn * 64 <= wm * 32 + 31);
+        double acc[4][8][2];
+        if (warp_active) {
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt) {
+                const int gi = tm0 + wm * 32 + mt * 8 + g;
+                const double* crow = A + (size_t)gi * ld;
+#pragma unroll
+                for (int nt = 0; nt < 8; ++nt) {
+                    const int gj = tn0 + wn * 64 + nt * 8 + 2 * t;
+                    double c0 = 0.0, c1 = 0.0;
+                    if (gi < M) {
+                        if (gj + 1 <= gi) {
+                            const double2 cv = *reinterpret_cast<const double2*>(crow + gj);
+                            c0 = cv.x; c1 = cv.y;
+                        } else if (gj <= gi) {
+                            c0 = crow[gj];
+                        }
+                    }
+                    acc[mt][nt][0] = -c0;
+                    acc[mt][nt][1] = -c1;
+                }
+            }
+        }
+        for (int kt = 0; kt < KT; ++kt) {
+            const uint32_t G = git + kt, sl = G % STAGES;
+            mbar_wait(bar_full + 8 * sl, (G / STAGES) & 1);
+            if (warp_active) {
+                const uint8_t* sa = ring_g + sl * STAGE_BYTES + offA;
+                const uint8_t* sb = ring_g + sl * STAGE_BYTES + (diag ? 0 : 2 * BOX_BYTES) + offB;
+                compute_box<0>(acc, sa, sb, xo0, xo1);
+                compute_box<0>(acc, sa + BOX_BYTES, sb + BOX_BYTES, xo0, xo1);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_empty + 8 * sl);
+        }
+        git += (uint32_t)KT;
+
+        if (!diag) {
+            // ---- S = D_ij - sum  ->  global (in place), read back as the A operand of  L_ij = S W_j^T ----
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt) {
+                const int gi = tm0 + wm * 32 + mt * 8 + g;
+                if (gi >= M) continue;
+                double* crow = A + (size_t)gi * ld;
+#pragma unroll
+                for (int nt = 0; nt < 8; ++nt) {
+                    const int gj = tn0 + wn * 64 + nt * 8 + 2 * t;           // gj + 1 < tn0 + 128 <= tm0 <= gi
+                    *reinterpret_cast<double2*>(crow + gj) = make_double2(-acc[mt][nt][0], -acc[mt][nt][1]);
+                }
+            }
+            fence_proxy_async();
+            mbar_arrive(bar_s);
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < 8; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
+            // X[r][cc] = sum_{p <= cc} S[r][p] W[cc][p], W lower triangular: zero blocks are skipped per 16 x 8 box
+            auto trsm_stage = [&](auto s4c) {
+                constexpr int S4 = decltype(s4c)::value;
+                const uint32_t G = git + S4, sl = G % STAGES;
+                mbar_wait(bar_full + 8 * sl, (G / STAGES) & 1);
+                const uint8_t* sa = ring_g + sl * STAGE_BYTES + offA;
+                const uint8_t* sb = ring_g + sl * STAGE_BYTES + 2 * BOX_BYTES + offB;
+                trsm_box<2 * S4>(acc, wn, sa, sb, xo0, xo1);
+                trsm_box<2 * S4 + 1>(acc, wn, sa + BOX_BYTES, sb + BOX_BYTES, xo0, xo1);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_empty + 8 * sl);
+            };
+            trsm_stage(std::integral_constant<int, 0>{});
+            trsm_stage(std::integral_constant<int, 1>{});
+            trsm_stage(std::integral_constant<int, 2>{});
+            trsm_stage(std::integral_constant<int, 3>{});
+            git += SPB;
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt) {
+                const int gi = tm0 + wm * 32 + mt * 8 + g;
+                if (gi >= M) continue;
+                double* crow = A + (size_t)gi * ld;
+#pragma unroll
+                for (int nt = 0; nt < 8; ++nt) {
+                    const int gj = tn0 + wn * 64 + nt * 8 + 2 * t;
+                    *reinterpret_cast<double2*>(crow + gj) = make_double2(acc[mt][nt][0], acc[mt][nt][1]);
+                }
+            }
+            __threadfence();
+            fence_proxy_async();
+            cons_sync();
+            if (tid == 0) st_release_gpu(flags_c + (size_t)i * T + j, a.epoch);
+        } else {
+            // ---- diagonal tile: S -> shared memory, L_jj = chol(S) and W_j = L_jj^-1 as 64 + 64 -------------
+            cons_sync();                                          // every warp is done with the ring
+            double* S11 = reinterpret_cast<double*>(ring_g);
+            double* S21 = S11 + 64 * potf2::SLDP;
+            double* S22 = S21 + 64 * potf2::SLDP;
+            double* W11 = S22 + 64 * potf2::SLDP;
+            double* W22 = W11 + 64 * potf2::SLDP;
+            double* sCol = W22 + 64 * potf2::SLDP;
+            double* sRinv = sCol + 64;
+            const int nloc = min(TB, M - tn0);                    // rows / columns of the block that exist
+            for (int idx = tid; idx < 64 * potf2::SLDP; idx += NCONS) { W11[idx] = 0.0; W22[idx] = 0.0; }
             if (warp_active) {
 #pragma unroll
                 for (int mt = 0; mt < 4; ++mt) {
-                    const int gi = tm0 + wm * 32 + mt * 8 + g;
-                    const double* crow = A + (size_t)gi * ld;
+                    const int R = wm * 32 + mt * 8 + g;
 #pragma unroll
-                    for (int nt = 0; nt < 8; ++nt) {
-                        const int gj = tn0 + wn * 64 + nt * 8 + 2 * t;
-                        double c0 = 0.0, c1 = 0.0;
-                        if (gi < M) {
-                            if (gj + 1 <= gi) {
-                                const double2 cv = *reinterpret_cast<const double2*>(crow + gj);
-                                c0 = cv.x; c1 = cv.y;
-                            } else if (gj <= gi) {
-                                c0 = crow[gj];
-                            }
+                    for (int nt = 0; nt < 8; ++nt)
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            const int Cc = wn * 64 + nt * 8 + 2 * t + e;
+                            double v = (Cc <= R) ? -acc[mt][nt][e] : 0.0;
+                            if (R >= nloc || Cc >= nloc) v = (R == Cc) ? 1.0 : 0.0;       // identity padding (ragged tile)
+                            double* dst = (R < 64) ? S11 + R * potf2::SLDP + Cc
+                                                   : (Cc < 64 ? S21 + (R - 64) * potf2::SLDP + Cc : S22 + (R - 64) * potf2::SLDP + (Cc - 64));
+                            if (R >= 64 || Cc < 64) *dst = v;
                         }
-                        acc[mt][nt][0] = -c0;
-                        acc[mt][nt][1] = -c1;
-                    }
                 }
             }
-            // one ring stage: 2 boxes x 2 chunk pairs x (12 LDS.128 + 64 DMMA) per warp
-            auto compute_stage = [&](uint32_t sl, bool b_is_a) {
-                const uint8_t* sa = ring_g + sl * STAGE_BYTES + offA;
-                const uint8_t* sb = ring_g + sl * STAGE_BYTES + (b_is_a ? 0 : 2 * BOX_BYTES) + offB;
+            if (tid == 0) sFail = 0;
+            cons_sync();
+            const int g64r = 16 * (warp & 3), g64c = 32 * (warp >> 2);     // gemm64 output block of this warp
+            double o[2][4][2];
+#pragma unroll 1
+            for (int hh = 0; hh < 2; ++hh) {
+                double* Sb = hh ? S22 : S11;
+                double* Wb = hh ? W22 : W11;
+                const int nrem = nloc - 64 * hh;
+                potf2::block64(Sb, Wb, sCol, sRinv, (nrem > potf2::HB) ? 2 : 1, lane, warp, tn0 + 64 * hh, &sFail, [] { cons_sync(); });
+                if (hh == 0) {
+                    potf2::gemm64(S21, W11, false, warp, lane, o);             // L21 = S21 W11^T
+                    cons_sync();
 #pragma unroll
-                for (int bx = 0; bx < 2; ++bx) {
+                    for (int mm = 0; mm < 2; ++mm)
 #pragma unroll
-                    for (int jj = 0; jj < 2; ++jj) {
-                        const int xo = jj ? xo1 : xo0;
-                        double2 af[4], bf[8];
+                        for (int nn = 0; nn < 4; ++nn) {
+                            const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t;
+                            S21[r * potf2::SLDP + cc] = o[mm][nn][0];
+                            S21[r * potf2::SLDP + cc + 1] = o[mm][nn][1];
+                            const int gi = tn0 + 64 + r;
+                            if (gi < M) *reinterpret_cast<double2*>(A + (size_t)gi * ld + tn0 + cc) = make_double2(o[mm][nn][0], o[mm][nn][1]);
+                        }
+                    cons_sync();
+                    potf2::gemm64(S21, S21, false, warp, lane, o);             // S22 -= L21 L21^T (lower part)
 #pragma unroll
-                        for (int mt = 0; mt < 4; ++mt) af[mt] = *reinterpret_cast<const double2*>(sa + bx * BOX_BYTES + mt * 1024 + xo);
+                    for (int mm = 0; mm < 2; ++mm)
 #pragma unroll
-                        for (int nt = 0; nt < 8; ++nt) bf[nt] = *reinterpret_cast<const double2*>(sb + bx * BOX_BYTES + nt * 1024 + xo);
-#pragma unroll
-                        for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-                            for (int nt = 0; nt < 8; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], af[mt].x, bf[nt].x);
-#pragma unroll
-                        for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-                            for (int nt = 0; nt < 8; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], af[mt].y, bf[nt].y);
-                    }
-                }
-            };
-            for (int kt = 0; kt < KT; ++kt) {
-                const uint32_t G = git + kt, sl = G % STAGES;
-                mbar_wait(bar_full + 8 * sl, (G / STAGES) & 1);
-                if (warp_active) compute_stage(sl, diag);
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar_empty + 8 * sl);
-            }
-
-            if (!diag) {
-                // ---- S = D_ij - sum  ->  global (in place), read back as the A operand of  L_ij = S W_j^T ----
-#pragma unroll
-                for (int mt = 0; mt < 4; ++mt) {
-                    const int gi = tm0 + wm * 32 + mt * 8 + g;
-                    if (gi >= M) continue;
-                    double* crow = A + (size_t)gi * ld;
-#pragma unroll
-                    for (int nt = 0; nt < 8; ++nt) {
-                        const int gj = tn0 + wn * 64 + nt * 8 + 2 * t;           // gj + 1 < tn0 + 128 <= tm0 <= gi
-                        *reinterpret_cast<double2*>(crow + gj) = make_double2(-acc[mt][nt][0], -acc[mt][nt][1]);
-                    }
-                }
-                fence_proxy_async();
-                mbar_arrive(bar_s);
-#pragma unroll
-                for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-                    for (int nt = 0; nt < 8; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
-                // X[r][cc] = sum_{p <= cc} S[r][p] W[cc][p]: columns 0..63 (wn = 0) need p < 64 only -> stages 0, 1
-                for (int s4 = 0; s4 < SPB; ++s4) {
-                    const uint32_t G = git + KT + s4, sl = G % STAGES;
-                    mbar_wait(bar_full + 8 * sl, (G / STAGES) & 1);
-                    if (wn == 1 || s4 < SPB / 2) compute_stage(sl, false);
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(bar_empty + 8 * sl);
-                }
-#pragma unroll
-                for (int mt = 0; mt < 4; ++mt) {
-                    const int gi = tm0 + wm * 32 + mt * 8 + g;
-                    if (gi >= M) continue;
-                    double* crow = A + (size_t)gi * ld;
-#pragma unroll
-                    for (int nt = 0; nt < 8; ++nt) {
-                        const int gj = tn0 + wn * 64 + nt * 8 + 2 * t;
-                        *reinterpret_cast<double2*>(crow + gj) = make_double2(acc[mt][nt][0], acc[mt][nt][1]);
-                    }
-                }
-                __threadfence();
-                fence_proxy_async();
-                cons_sync();
-                if (tid == 0) st_release_gpu(flags_c + (size_t)i * T + j, a.epoch);
-            } else {
-                // ---- diagonal tile: S -> shared memory, L_jj = chol(S) and W_j = L_jj^-1 as 64 + 64 -------------
-                cons_sync();                                          // every warp is done with the ring
-                double* S11 = reinterpret_cast<double*>(ring_g);
-                double* S21 = S11 + 64 * potf2::SLDP;
-                double* S22 = S21 + 64 * potf2::SLDP;
-                double* W11 = S22 + 64 * potf2::SLDP;
-                double* W22 = W11 + 64 * potf2::SLDP;
-                double* sCol = W22 + 64 * potf2::SLDP;
-                double* sRinv = sCol + 64;
-                const int nloc = min(TB, M - tn0);                    // rows / columns of the block that exist
-                for (int idx = tid; idx < 64 * potf2::SLDP; idx += NCONS) { W11[idx] = 0.0; W22[idx] = 0.0; }
-                if (warp_active) {
-#pragma unroll
-                    for (int mt = 0; mt < 4; ++mt) {
-                        const int R = wm * 32 + mt * 8 + g;
-#pragma unroll
-                        for (int nt = 0; nt < 8; ++nt)
+                        for (int nn = 0; nn < 4; ++nn)
 #pragma unroll
                             for (int e = 0; e < 2; ++e) {
-                                const int Cc = wn * 64 + nt * 8 + 2 * t + e;
-                                double v = (Cc <= R) ? -acc[mt][nt][e] : 0.0;
-                                if (R >= nloc || Cc >= nloc) v = (R == Cc) ? 1.0 : 0.0;       // identity padding (ragged tile)
-                                double* dst = (R < 64) ? S11 + R * potf2::SLDP + Cc
-                                                       : (Cc < 64 ? S21 + (R - 64) * potf2::SLDP + Cc : S22 + (R - 64) * potf2::SLDP + (Cc - 64));
-                                if (R >= 64 || Cc < 64) *dst = v;
+                                const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t + e;
+                                if (cc <= r && 64 + r < nloc) S22[r * potf2::SLDP + cc] -= o[mm][nn][e];
                             }
-                    }
-                }
-                if (tid == 0) sFail = 0;
-                cons_sync();
-                const int g64r = 16 * (warp & 3), g64c = 32 * (warp >> 2);     // gemm64 output block of this warp
-                double o[2][4][2];
-#pragma unroll 1
-                for (int hh = 0; hh < 2; ++hh) {
-                    double* Sb = hh ? S22 : S11;
-                    double* Wb = hh ? W22 : W11;
-                    const int nrem = nloc - 64 * hh;
-                    potf2::block64(Sb, Wb, sCol, sRinv, (nrem > potf2::HB) ? 2 : 1, lane, warp, tn0 + 64 * hh, &sFail, [] { cons_sync(); });
-                    if (hh == 0) {
-                        potf2::gemm64(S21, W11, false, warp, lane, o);             // L21 = S21 W11^T
-                        cons_sync();
-#pragma unroll
-                        for (int mm = 0; mm < 2; ++mm)
-#pragma unroll
-                            for (int nn = 0; nn < 4; ++nn) {
-                                const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t;
-                                S21[r * potf2::SLDP + cc] = o[mm][nn][0];
-                                S21[r * potf2::SLDP + cc + 1] = o[mm][nn][1];
-                                const int gi = tn0 + 64 + r;
-                                if (gi < M) *reinterpret_cast<double2*>(A + (size_t)gi * ld + tn0 + cc) = make_double2(o[mm][nn][0], o[mm][nn][1]);
-                            }
-                        cons_sync();
-                        potf2::gemm64(S21, S21, false, warp, lane, o);             // S22 -= L21 L21^T (lower part)
-#pragma unroll
-                        for (int mm = 0; mm < 2; ++mm)
-#pragma unroll
-                            for (int nn = 0; nn < 4; ++nn)
-#pragma unroll
-                                for (int e = 0; e < 2; ++e) {
-                                    const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t + e;
-                                    if (cc <= r && 64 + r < nloc) S22[r * potf2::SLDP + cc] -= o[mm][nn][e];
-                                }
-                        cons_sync();
-                    }
-                }
-                potf2::gemm64(S21, W11, true, warp, lane, o);                      // Tm = L21 W11
-                cons_sync();
-#pragma unroll
-                for (int mm = 0; mm < 2; ++mm)
-#pragma unroll
-                    for (int nn = 0; nn < 4; ++nn) {
-                        const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t;
-                        S21[r * potf2::SLDP + cc] = o[mm][nn][0];
-                        S21[r * potf2::SLDP + cc + 1] = o[mm][nn][1];
-                    }
-                cons_sync();
-                potf2::gemm64(W22, S21, true, warp, lane, o);                      // W21 = -W22 Tm
-                double* Wg = a.Wbuf + ((size_t)c * T + j) * TB * TB;
-#pragma unroll
-                for (int mm = 0; mm < 2; ++mm)
-#pragma unroll
-                    for (int nn = 0; nn < 4; ++nn) {
-                        const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t;
-                        *reinterpret_cast<double2*>(Wg + (size_t)(64 + r) * TB + cc) = make_double2(-o[mm][nn][0], -o[mm][nn][1]);
-                    }
-                // L11, L22 -> the matrix (lower triangle only); W11, 0, W22 -> Wbuf
-                for (int idx = tid; idx < 64 * 64; idx += NCONS) {
-                    const int r = idx >> 6, cc = idx & 63;
-                    if (cc <= r) {
-                        if (tn0 + r < M) A[(size_t)(tn0 + r) * ld + tn0 + cc] = S11[r * potf2::SLDP + cc];
-                        if (tn0 + 64 + r < M) A[(size_t)(tn0 + 64 + r) * ld + tn0 + 64 + cc] = S22[r * potf2::SLDP + cc];
-                    }
-                    Wg[(size_t)r * TB + cc] = W11[r * potf2::SLDP + cc];
-                    Wg[(size_t)r * TB + 64 + cc] = 0.0;
-                    Wg[(size_t)(64 + r) * TB + 64 + cc] = W22[r * potf2::SLDP + cc];
-                }
-                __threadfence();
-                fence_proxy_async();
-                cons_sync();
-                if (tid == 0) {
-                    if (sFail != 0 && a.info != nullptr && a.info[c] == 0) a.info[c] = sFail;
-                    st_release_gpu(flags_c + (size_t)j * T + j, a.epoch);
+                    cons_sync();
                 }
             }
-            git += (uint32_t)(KT + KE);
-            __syncthreads();
-            if (tid == 0) sTicket = atomicAdd(a.ticket, 1u) - a.ticket_base;
-            __syncthreads();
+            potf2::gemm64(S21, W11, true, warp, lane, o);                      // Tm = L21 W11
+            cons_sync();
+#pragma unroll
+            for (int mm = 0; mm < 2; ++mm)
+#pragma unroll
+                for (int nn = 0; nn < 4; ++nn) {
+                    const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t;
+                    S21[r * potf2::SLDP + cc] = o[mm][nn][0];
+                    S21[r * potf2::SLDP + cc + 1] = o[mm][nn][1];
+                }
+            cons_sync();
+            potf2::gemm64(W22, S21, true, warp, lane, o);                      // W21 = -W22 Tm
+            double* Wg = a.Wbuf + ((size_t)c * T + j) * TB * TB;
+#pragma unroll
+            for (int mm = 0; mm < 2; ++mm)
+#pragma unroll
+                for (int nn = 0; nn < 4; ++nn) {
+                    const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t;
+                    *reinterpret_cast<double2*>(Wg + (size_t)(64 + r) * TB + cc) = make_double2(-o[mm][nn][0], -o[mm][nn][1]);
+                }
+            // L11, L22 -> the matrix (lower triangle only); W11, 0, W22 -> Wbuf
+            for (int idx = tid; idx < 64 * 64; idx += NCONS) {
+                const int r = idx >> 6, cc = idx & 63;
+                if (cc <= r) {
+                    if (tn0 + r < M) A[(size_t)(tn0 + r) * ld + tn0 + cc] = S11[r * potf2::SLDP + cc];
+                    if (tn0 + 64 + r < M) A[(size_t)(tn0 + 64 + r) * ld + tn0 + 64 + cc] = S22[r * potf2::SLDP + cc];
+                }
+                Wg[(size_t)r * TB + cc] = W11[r * potf2::SLDP + cc];
+                Wg[(size_t)r * TB + 64 + cc] = 0.0;
+                Wg[(size_t)(64 + r) * TB + 64 + cc] = W22[r * potf2::SLDP + cc];
+            }
+            __threadfence();
+            fence_proxy_async();
+            cons_sync();
+            if (tid == 0) {
+                if (sFail != 0 && a.info != nullptr && a.info[c] == 0) a.info[c] = sFail;
+                st_release_gpu(flags_c + (size_t)j * T + j, a.epoch);
+            }
+            if (lane == 0) mbar_arrive(bar_d);                    // the ring may be refilled
         }
     }
 }
@@ -497,7 +537,7 @@ int bdk_potrf_tiles(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t*
     a.total = (unsigned)total64;
     a.info = info;
     const unsigned grid = (a.total < (unsigned)ctx->num_sms) ? a.total : (unsigned)ctx->num_sms;
-    ctx->tile_ticket_base += a.total + grid;          // every CTA draws exactly one ticket beyond the last tile
+    ctx->tile_ticket_base += a.total + grid;          // every CTA's producer draws exactly one ticket beyond the last tile
     BD_LAUNCH(ctx, k_potrf_tiles, dim3(grid), dim3(NTHREADS), TILE_SMEM, *reinterpret_cast<const CUtensorMap*>(&ctx->tile_maps[0]),
               *reinterpret_cast<const CUtensorMap*>(&ctx->tile_maps[1]), a);
     return 0;
