@@ -104,10 +104,13 @@ __device__ __forceinline__ void decode_ticket(unsigned tk, int C, int T, int& j,
 
 // One 128 x 16 box of both operands: 2 chunk pairs x (4 + (8 - NTLO) LDS.128, 2 x 4 x (8 - NTLO) DMMA) per warp.  NTLO > 0 skips
 // the first n-tiles (the S W^T pass: W is lower triangular, column block nt of the warp needs p <= its last column only).
-template <int NTLO>
+// NTHI >= 0 instead keeps, for the m-tile mt, only the n-tiles nt <= NTHI + mt (a 32 x 64 block that the diagonal of a
+// diagonal tile crosses: everything right of it is never used).
+template <int NTLO, int NTHI = 8>
 __device__ __forceinline__ void compute_box(double (&acc)[4][8][2], const uint8_t* __restrict__ sa, const uint8_t* __restrict__ sb,
                                             const int xo0, const int xo1)
 {
+    constexpr int NTE = (NTHI + 3 < 7) ? NTHI + 4 : 8;         // n-tiles any m-tile needs
 #pragma unroll
     for (int jj = 0; jj < 2; ++jj) {
         const int xo = jj ? xo1 : xo0;
@@ -115,15 +118,17 @@ __device__ __forceinline__ void compute_box(double (&acc)[4][8][2], const uint8_
 #pragma unroll
         for (int mt = 0; mt < 4; ++mt) af[mt] = *reinterpret_cast<const double2*>(sa + mt * 1024 + xo);
 #pragma unroll
-        for (int nt = NTLO; nt < 8; ++nt) bf[nt] = *reinterpret_cast<const double2*>(sb + nt * 1024 + xo);
+        for (int nt = NTLO; nt < NTE; ++nt) bf[nt] = *reinterpret_cast<const double2*>(sb + nt * 1024 + xo);
 #pragma unroll
         for (int mt = 0; mt < 4; ++mt)
 #pragma unroll
-            for (int nt = NTLO; nt < 8; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], af[mt].x, bf[nt].x);
+            for (int nt = NTLO; nt < NTE; ++nt)
+                if (nt <= NTHI + mt) dmma884(acc[mt][nt][0], acc[mt][nt][1], af[mt].x, bf[nt].x);
 #pragma unroll
         for (int mt = 0; mt < 4; ++mt)
 #pragma unroll
-            for (int nt = NTLO; nt < 8; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], af[mt].y, bf[nt].y);
+            for (int nt = NTLO; nt < NTE; ++nt)
+                if (nt <= NTHI + mt) dmma884(acc[mt][nt][0], acc[mt][nt][1], af[mt].y, bf[nt].y);
     }
 }
 
@@ -150,7 +155,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_potrf_tiles(const __grid_consta
     __shared__ int sFail;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wm = warp & 3, wn = (warp >> 2) & 1;
     const int g = lane >> 2, t = lane & 3;
     const uint32_t ring = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* ring_g = smem_raw + (ring - smem_u32(smem_raw));
@@ -253,7 +257,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_potrf_tiles(const __grid_consta
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(REGS_CONSUMER));
     // fragment addressing inside a 128 x 16 box: row r at r * 128 bytes, logical 16-byte chunk q at (q ^ (r & 7)) * 16
     const int xo0 = ((2 * t) ^ g) * 16, xo1 = ((2 * t + 1) ^ g) * 16;
-    const int offA = (wm * 32 + g) * 128, offB = (wn * 64 + g) * 128;
+    const int wm_off = warp & 3, wn_off = (warp >> 2) & 1;
+    // Diagonal tiles need the lower triangle only: of the eight 32 x 64 warp blocks two lie above the diagonal, two are
+    // full and four are crossed by it (10 or 26 of their 32 DMMA tiles are needed).  The six blocks are dealt to the warps
+    // so that every sub-partition (warp & 3) gets the same work: {A, F}, {B, E}, {C}, {D} = 36, 36, 32, 32 DMMA tiles per k-step
+    // (all eight blocks on their home warps would cost 64).  pattern 0: idle, 1: n-tile <= m-tile, 2: n-tile <= m-tile + 4, 3: full.
+    const int wm_dg = (warp < 4) ? warp : (warp == 4 ? 3 : 2), wn_dg = (warp == 4 || warp == 5) ? 1 : 0;
+    const int pat_dg = (warp == 0 || warp == 5) ? 1 : (warp == 1 || warp == 4) ? 2 : (warp < 4) ? 3 : 0;
     uint32_t git = 0;                                  // ring stages consumed so far
     for (uint32_t n = 0;; ++n) {
         const uint32_t qs = n % QD;
@@ -269,8 +279,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_potrf_tiles(const __grid_consta
         double* A = a.A + (size_t)c * a.stride;
         int* flags_c = a.flags + (size_t)c * T * T;
         const int tm0 = i * TB, tn0 = j * TB;
-        // this warp's 32 x 64 block lies entirely above the diagonal of a diagonal tile -> no arithmetic
-        const bool warp_active = !diag || (wn * 64 <= wm * 32 + 31);
+        const int wm = diag ? wm_dg : wm_off, wn = diag ? wn_dg : wn_off;       // this warp's 32 x 64 block of the tile
+        const int offA = (wm * 32 + g) * 128, offB = (wn * 64 + g) * 128;
+        const bool warp_active = !diag || pat_dg != 0;
         double acc[4][8][2];
         if (warp_active) {
 #pragma unroll
@@ -294,18 +305,27 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_potrf_tiles(const __grid_consta
                 }
             }
         }
-        for (int kt = 0; kt < KT; ++kt) {
-            const uint32_t G = git + kt, sl = G % STAGES;
-            mbar_wait(bar_full + 8 * sl, (G / STAGES) & 1);
-            if (warp_active) {
-                const uint8_t* sa = ring_g + sl * STAGE_BYTES + offA;
-                const uint8_t* sb = ring_g + sl * STAGE_BYTES + (diag ? 0 : 2 * BOX_BYTES) + offB;
-                compute_box<0>(acc, sa, sb, xo0, xo1);
-                compute_box<0>(acc, sa + BOX_BYTES, sb + BOX_BYTES, xo0, xo1);
+        // K loop; pc = std::integral_constant of the block pattern (3 = all 32 DMMA tiles)
+        auto k_loop = [&](auto pc, const int b_off) {
+            constexpr int NTHI = (decltype(pc)::value == 1) ? 0 : (decltype(pc)::value == 2) ? 4 : 8;
+            for (int kt = 0; kt < KT; ++kt) {
+                const uint32_t G = git + kt, sl = G % STAGES;
+                mbar_wait(bar_full + 8 * sl, (G / STAGES) & 1);
+                if constexpr (decltype(pc)::value != 0) {
+                    const uint8_t* sa = ring_g + sl * STAGE_BYTES + offA;
+                    const uint8_t* sb = ring_g + sl * STAGE_BYTES + b_off + offB;
+                    compute_box<0, NTHI>(acc, sa, sb, xo0, xo1);
+                    compute_box<0, NTHI>(acc, sa + BOX_BYTES, sb + BOX_BYTES, xo0, xo1);
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_empty + 8 * sl);
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar_empty + 8 * sl);
-        }
+        };
+        if (!diag) k_loop(std::integral_constant<int, 3>{}, 2 * BOX_BYTES);
+        else if (pat_dg == 3) k_loop(std::integral_constant<int, 3>{}, 0);          // B operand = the A boxes (rows j = rows i)
+        else if (pat_dg == 2) k_loop(std::integral_constant<int, 2>{}, 0);
+        else if (pat_dg == 1) k_loop(std::integral_constant<int, 1>{}, 0);
+        else k_loop(std::integral_constant<int, 0>{}, 0);
         git += (uint32_t)KT;
 
         if (!diag) {
