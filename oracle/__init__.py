@@ -45,7 +45,7 @@ def build(force: bool = False) -> str:
 class _Params(C.Structure):
     _fields_ = [("n_rods", C.c_int32), ("b", C.c_double), ("hstar", C.c_double), ("a", C.c_double),
                 ("K", C.c_double), ("dt", C.c_double), ("kappa", C.c_double * 9),
-                ("seed", C.c_uint64), ("noise_kind", C.c_int32)]
+                ("seed", C.c_uint64), ("noise_kind", C.c_int32), ("spring_kind", C.c_int32), ("nu", C.c_double)]
 
 
 class _Trace(C.Structure):
@@ -63,6 +63,8 @@ def lib():
         _lib.orc_u01.argtypes = [C.c_uint64]
         for name in ("orc_cholesky", "orc_finish_step", "orc_step", "orc_step_ensemble", "orc_num_threads"):
             getattr(_lib, name).restype = C.c_int32
+        _lib.orc_spring_coeff.restype = C.c_double
+        _lib.orc_implicit_length.restype = C.c_double
     return _lib
 
 
@@ -78,6 +80,8 @@ class Params:
     kappa: np.ndarray = field(default_factory=lambda: np.zeros((3, 3)))
     seed: int = 0
     noise_kind: int = 0
+    spring_kind: int = 0     # 0 Fraenkel rod (Eq. 3), 1 Cohen-Pade spring (Eq. 4)
+    nu: float = 0.0          # Kuhn steps per spring (kind 1)
 
     def c(self) -> _Params:
         p = _Params()
@@ -92,6 +96,8 @@ class Params:
             p.kappa[i] = float(k[i])
         p.seed = int(self.seed)
         p.noise_kind = int(self.noise_kind)
+        p.spring_kind = int(self.spring_kind)
+        p.nu = float(self.nu)
         return p
 
     @property
@@ -146,6 +152,18 @@ def init_random_walk(n_rods: int, b: float, init_seed: int, chains) -> np.ndarra
         lib().orc_init_random_walk(C.c_int32(n_rods), C.c_double(b), C.c_uint64(init_seed),
                                    C.c_uint64(c), _ptr(r[i]))
     return r
+
+
+def spring_coeff(p: Params, q: float) -> float:
+    """T = spring_coeff(|Q|) * Q (Eq. 3 or Eq. 4)."""
+    cp = p.c()
+    return float(lib().orc_spring_coeff(C.byref(cp), C.c_double(q)))
+
+
+def implicit_length(p: Params, Yn: float) -> float:
+    """|Q'| from |Y| (Eq. 17, or the Cohen-Pade cubic)."""
+    cp = p.c()
+    return float(lib().orc_implicit_length(C.byref(cp), C.c_double(Yn)))
 
 
 def spring_tensions(p: Params, r) -> np.ndarray:

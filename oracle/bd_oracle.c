@@ -151,15 +151,54 @@ void orc_init_random_walk(int32_t n_rods, double b, uint64_t init_seed, uint64_t
 /* ---------------------------------------------------------------------------------------
  * Eq. 3: T_k = K (|Q_k| - b)/|Q_k| Q_k  (paper: b = 1).
  * ------------------------------------------------------------------------------------- */
+double orc_spring_coeff(const orc_params *p, double q)
+{
+    if (p->spring_kind == 1) {
+        /* Eq. 4: |F| = (alpha r^ - beta r^^3)/(1 - r^^2), alpha = 3, beta = 1,
+         * r^ = |Q|/(nu b) the fractional extension; force in units of kT/b (lengths in b,
+         * DESIGN.md reading B4), direction along Q:  T = (|F|/b) Q/|Q|.                      */
+        double x = q / (p->nu * p->b);
+        double F = (3.0 * x - x * x * x) / (1.0 - x * x);
+        return (F / p->b) / q;
+    }
+    return p->K * (q - p->b) / q;                      /* Eq. 3 */
+}
+
 void orc_spring_tensions(const orc_params *p, const double *r, double *T)
 {
     for (int32_t k = 0; k < p->n_rods; ++k) {
         double Q[3];
         for (int d = 0; d < 3; ++d) Q[d] = r[3 * (k + 1) + d] - r[3 * k + d];
         double q = sqrt(Q[0] * Q[0] + Q[1] * Q[1] + Q[2] * Q[2]);
-        double c = p->K * (q - p->b) / q;
+        double c = orc_spring_coeff(p, q);
         for (int d = 0; d < 3; ++d) T[3 * k + d] = c * Q[d];
     }
+}
+
+/* ---------------------------------------------------------------------------------------
+ * Semi-implicit link length.  Eq. 13 with D_ii = I (Eq. 7): Y = Q' + 2 dt T(Q'), T parallel to
+ * Q', so |Y| = |Q'| + 2 dt |T(|Q'|)|.
+ *  Fraenkel rod (Eq. 3):  |Q'| = (2 dt K b + |Y|)/(2 dt K + 1)                       (Eq. 17)
+ *  Cohen-Pade spring (Eq. 4), x = |Q'|/(nu b), y = |Y|/(nu b), c = 2 dt/(nu b^2):
+ *      y = x + c (3x - x^3)/(1 - x^2)   <=>   (1 + c) x^3 - y x^2 - (1 + 3c) x + y = 0,
+ *  f(0) = y >= 0 and f(1) = -2c < 0: exactly one root in [0, 1) (finite extensibility); found
+ *  by plain bisection (200 halvings: to the last bit).  The paper states the scheme for the
+ *  Fraenkel spring only and refers to its ref. [27] for the rest (reading B4).
+ * ------------------------------------------------------------------------------------- */
+double orc_implicit_length(const orc_params *p, double Yn)
+{
+    if (p->spring_kind == 1) {
+        double L = p->nu * p->b;
+        double y = Yn / L, c = 2.0 * p->dt / (p->nu * p->b * p->b);
+        double lo = 0.0, hi = 1.0;
+        for (int it = 0; it < 200; ++it) {
+            double x = 0.5 * (lo + hi);
+            double f = ((1.0 + c) * x - y) * x * x - (1.0 + 3.0 * c) * x + y;
+            if (f > 0.0) lo = x; else hi = x;
+        }
+        return 0.5 * (lo + hi) * L;
+    }
+    return (2.0 * p->dt * p->K * p->b + Yn) / (2.0 * p->dt * p->K + 1.0);
 }
 
 /* Eq. 1 net spring term (F^S_{i+1} - F^S_i) and Eq. 22:
@@ -317,7 +356,7 @@ int32_t orc_finish_step(const orc_params *p, const double *r, const double *T, c
             Y[d] = Q + (u[3 * (k + 1) + d] - u[3 * k + d]) + 2.0 * p->dt * T[3 * k + d];
         }
         double Yn = sqrt(Y[0] * Y[0] + Y[1] * Y[1] + Y[2] * Y[2]);
-        double qn = (2.0 * p->dt * p->K * p->b + Yn) / (2.0 * p->dt * p->K + 1.0);
+        double qn = orc_implicit_length(p, Yn);          /* Eq. 17 (or the Cohen-Pade cubic) */
         double scale = qn / Yn;
         if (!(Yn > 0.0) || !isfinite(scale)) info = M + 1;
         for (int d = 0; d < 3; ++d) {
@@ -424,7 +463,7 @@ void orc_observables_chain(const orc_params *p, const double *r, double obs[ORC_
         double Q[3], T[3];
         for (int d = 0; d < 3; ++d) Q[d] = r[3 * (k + 1) + d] - r[3 * k + d];
         double q = sqrt(Q[0] * Q[0] + Q[1] * Q[1] + Q[2] * Q[2]);
-        double c = p->K * (q - p->b) / q;
+        double c = orc_spring_coeff(p, q);
         for (int d = 0; d < 3; ++d) T[d] = c * Q[d];
         S[0] += T[0] * Q[0]; S[1] += T[1] * Q[1]; S[2] += T[2] * Q[2];
         S[3] += T[0] * Q[1]; S[4] += T[0] * Q[2]; S[5] += T[1] * Q[2];

@@ -42,6 +42,8 @@ typedef struct {
     double   kappa[9];    /* row-major, v = kappa . r (Eq. 5)            */
     uint64_t seed;        /* Philox key                                                  */
     int32_t  noise_kind;  /* 0 Gaussian sqrt(2dt) g ; 1 uniform sqrt(6dt) n (Eq. 2)      */
+    int32_t  spring_kind; /* 0 Fraenkel rod (Eq. 3) ; 1 Cohen-Pade spring (Eq. 4)        */
+    double   nu;          /* Kuhn steps per spring (Eq. 4: r^ = |Q| / (nu b)); kind 1    */
 } orc_params;
 
 /* optional per-step intermediates; any pointer may be NULL */
@@ -69,6 +71,11 @@ void   orc_noise_dW(const orc_params *p, uint64_t chain, uint64_t step, double *
 void   orc_init_random_walk(int32_t n_rods, double b, uint64_t init_seed, uint64_t chain, double *r);
 
 /* --- forces ------------------------------------------------------------------------------ */
+/* spring law: T = orc_spring_coeff(p, |Q|) * Q  (Eq. 3, or Eq. 4 with alpha = 3, beta = 1)      */
+double orc_spring_coeff(const orc_params *p, double q);
+/* semi-implicit link length |Q'| from |Y| (Eq. 17 for the Fraenkel rod; for the Cohen-Pade spring
+ * the root in [0, nu b) of Eq. 13 written with Eq. 4 -- a cubic, reading B4)          */
+double orc_implicit_length(const orc_params *p, double Yn);
 void   orc_spring_tensions(const orc_params *p, const double *r, double *T);
 void   orc_bead_forces(int32_t n_rods, const double *T, double *F);
 
