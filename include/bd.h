@@ -61,6 +61,11 @@ typedef struct {
                               chain_id0 + c, so an ensemble sharded over GPUs is reproducible)    */
     int32_t  noise_kind;   /* 0: Gaussian, dW = sqrt(2 dt) g (Philox + Box-Muller);
                               1: the paper's uniform law, dW = sqrt(6 dt) n, n in [-1,1] (Eq. 2)  */
+    int32_t  spring_kind;  /* 0: Fraenkel rod, Eq. 3 (the bead-rod chain of the paper);
+                              1: Cohen-Pade spring, Eq. 4 with alpha = 3, beta = 1 (:78-82), the
+                              bead-spring comparison model (:305-307); K is then unused             */
+    double   nu;           /* Kuhn steps per spring (Eq. 4: fractional extension |Q| / (nu b));
+                              > 0 required when spring_kind = 1                                    */
 } bd_params;
 
 /* Create a context bound to cuda_stream (a cudaStream_t passed as void*, NULL = default stream).

@@ -23,7 +23,8 @@ ERR_CUDA, ERR_WORKSPACE, ERR_ALLOC = -100, -101, -102
 class bd_params(C.Structure):
     _fields_ = [("n_rods", C.c_int32), ("n_chains", C.c_int32), ("b", C.c_double), ("hstar", C.c_double),
                 ("a", C.c_double), ("K", C.c_double), ("dt", C.c_double), ("kappa", C.c_double * 9),
-                ("seed", C.c_uint64), ("chain_id0", C.c_uint64), ("noise_kind", C.c_int32)]
+                ("seed", C.c_uint64), ("chain_id0", C.c_uint64), ("noise_kind", C.c_int32), ("spring_kind", C.c_int32),
+                ("nu", C.c_double)]
 
 
 EXPORTS = ("bd_create", "bd_destroy", "bd_workspace_bytes", "bd_set_workspace", "bd_set_flow",
@@ -100,7 +101,8 @@ class BD:
 
     def __init__(self, n_rods: int, n_chains: int, dt: float, hstar: float = 0.25, b: float = 1.0,
                  a: float = -1.0, K: float = -1.0, kappa=None, seed: int = 0, chain_id0: int = 0,
-                 noise_kind: int = 0, stream: torch.cuda.Stream | None = None, device: str = "cuda:0"):
+                 noise_kind: int = 0, spring_kind: int = 0, nu: float = 0.0, stream: torch.cuda.Stream | None = None,
+                 device: str = "cuda:0"):
         self.lib = load_library()
         if not torch.cuda.is_available():
             raise RuntimeError("libbd needs a CUDA device (B200): there is no CPU fallback")
@@ -114,6 +116,7 @@ class BD:
         for i in range(9):
             p.kappa[i] = float(k[i])
         p.seed, p.chain_id0, p.noise_kind = int(seed), int(chain_id0), int(noise_kind)
+        p.spring_kind, p.nu = int(spring_kind), float(nu)
         self.params = p
         self.N, self.C, self.M = int(n_rods), int(n_chains), 3 * (int(n_rods) + 1)
         self._ctx = C.c_void_p()

@@ -46,6 +46,8 @@ int bd_create(const bd_params* params, void* cuda_stream, bd_ctx** out)
     if (p.hstar * p.b > p.a * (1.0 + 1e-12)) return -1;    // h*/a > 1: D not guaranteed positive definite (A3)
     if (!(p.K > 0.0)) p.K = 1.0 / p.dt;                    // reading A6: K* dt = 1
     if (p.noise_kind != 0 && p.noise_kind != 1) return -1;
+    if (p.spring_kind != 0 && p.spring_kind != 1) return -1;
+    if (p.spring_kind == 1 && !(p.nu > 0.0 && std::isfinite(p.nu))) return -1;
     for (int i = 0; i < 9; ++i)
         if (!std::isfinite(p.kappa[i])) return -1;
     if ((int64_t)3 * ((int64_t)p.n_rods + 1) > (int64_t)1 << 20) return -1;

@@ -102,6 +102,57 @@ __device__ __forceinline__ double warp_max(double x)
     return x;
 }
 
+// Spring law of the connectors (a1, a7).  kind 0: Fraenkel rod, T = K (|Q| - b)/|Q| Q (Eq. 3);
+// kind 1: Cohen-Pade spring, |T| = (3 x - x^3)/(1 - x^2) / b with x = |Q| / (nu b) (Eq. 4, :78-82, alpha = 3, beta = 1;
+// DESIGN.md reading B4 for the units).
+struct SpringLaw {
+    int kind;
+    double K, b, dt;
+    double inv_L, L, inv_b, c;       // kind 1: L = nu b (full extension), c = 2 dt / (nu b^2)
+};
+inline SpringLaw make_spring_law(const bd_params& p)
+{
+    SpringLaw s;
+    s.kind = p.spring_kind; s.K = p.K; s.b = p.b; s.dt = p.dt;
+    s.L = (p.spring_kind == 1) ? p.nu * p.b : 1.0;
+    s.inv_L = 1.0 / s.L; s.inv_b = 1.0 / p.b;
+    s.c = (p.spring_kind == 1) ? 2.0 * p.dt / (p.nu * p.b * p.b) : 0.0;
+    return s;
+}
+// tension = spring_coeff(q) * Q, q = |Q|
+__device__ __forceinline__ double spring_coeff(const SpringLaw& s, double q)
+{
+    if (s.kind == 1) {
+        const double x = q * s.inv_L;
+        return ((3.0 * x - x * x * x) / (1.0 - x * x)) * s.inv_b / q;
+    }
+    return s.K * (q - s.b) / q;
+}
+// semi-implicit link length |Q'| from |Y|: Eq. 17 (:154) for the rod; for the Cohen-Pade spring the root in [0, 1) of
+// (1 + c) x^3 - y x^2 - (1 + 3c) x + y = 0 (Eq. 13 written with Eq. 4; f(0) = y >= 0, f(1) = -2c < 0), bracketed by
+// bisection and finished by Newton steps that are kept inside the bracket.
+__device__ __forceinline__ double implicit_length(const SpringLaw& s, double Yn)
+{
+    if (s.kind == 1) {
+        const double y = Yn * s.inv_L, c = s.c;
+        double lo = 0.0, hi = 1.0;
+        auto f = [&](double x) { return ((1.0 + c) * x - y) * x * x - (1.0 + 3.0 * c) * x + y; };
+        for (int it = 0; it < 40; ++it) {
+            const double x = 0.5 * (lo + hi);
+            if (f(x) > 0.0) lo = x; else hi = x;
+        }
+        double x = 0.5 * (lo + hi);
+        for (int it = 0; it < 3; ++it) {
+            const double df = (3.0 * (1.0 + c) * x - 2.0 * y) * x - (1.0 + 3.0 * c);
+            const double xn = x - f(x) / df;
+            if (xn > lo && xn < hi) x = xn;
+        }
+        return x * s.L;
+    }
+    const double tdk = 2.0 * s.dt * s.K;
+    return (tdk * s.b + Yn) / (tdk + 1.0);
+}
+
 // RPY off-diagonal block coefficients (Eqs. 8-9): block = cI*I + cRR*Rv Rv^T with
 // Rv = (r_i - r_j)/b, a_s = a/b, inv_a = 1/a_s.  One rsqrt, no divisions: 1/R = rsqrt(R^2).
 __device__ __forceinline__ void rpy_coeffs(double R2, double hstar, double a_s, double inv_a, double& cI, double& cRR)

@@ -38,7 +38,8 @@ constexpr int CS_STAGES = 2;              // ring stages
 
 struct ChainStepParams {
     int N, C;
-    double b, hstar, a_s, inv_a, inv_b, K, dt;
+    double b, hstar, a_s, inv_a, inv_b, dt;
+    SpringLaw sl;
     double kap[9];
     uint64_t seed, chain0, first_step;
     int n_steps, noise_kind;
@@ -114,7 +115,7 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                     if (k < 0 || k >= N) continue;
                     const double qx = sR[3 * k + 3] - sR[3 * k], qy = sR[3 * k + 4] - sR[3 * k + 1], qz = sR[3 * k + 5] - sR[3 * k + 2];
                     const double q = sqrt(qx * qx + qy * qy + qz * qz);
-                    const double cf = P.K * (q - P.b) / q;
+                    const double cf = spring_coeff(P.sl, q);
                     double* T = side ? Tr : Tl;
                     T[0] = cf * qx; T[1] = cf * qy; T[2] = cf * qz;
                 }
@@ -385,7 +386,6 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
             }
             bool bad = false;
             {
-                const double tdk = 2.0 * P.dt * P.K;
                 double carry[3] = {0.0, 0.0, 0.0}, sum[3] = {0.0, 0.0, 0.0};
                 for (int base = 0; base < N; base += CS_THREADS) {
                     const int k = base + tid;
@@ -396,7 +396,7 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                         for (int d = 0; d < 3; ++d) { ra[d] = sR[3 * k + d]; rb[d] = sR[3 * k + 3 + d]; }
                         const double Q[3] = {rb[0] - ra[0], rb[1] - ra[1], rb[2] - ra[2]};
                         const double qn = sqrt(Q[0] * Q[0] + Q[1] * Q[1] + Q[2] * Q[2]);
-                        const double tc = P.K * (qn - P.b) / qn;
+                        const double tc = spring_coeff(P.sl, qn);
 #pragma unroll
                         for (int d = 0; d < 3; ++d) {
                             const double fa = P.kap[3 * d] * ra[0] + P.kap[3 * d + 1] * ra[1] + P.kap[3 * d + 2] * ra[2];
@@ -406,7 +406,7 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                             Y[d] = Q[d] + (ub - ua) + 2.0 * P.dt * (tc * Q[d]);
                         }
                         const double Yn = sqrt(Y[0] * Y[0] + Y[1] * Y[1] + Y[2] * Y[2]);
-                        const double scale = ((tdk * P.b + Yn) / (tdk + 1.0)) / Yn;
+                        const double scale = implicit_length(P.sl, Yn) / Yn;
                         if (!(Yn > 0.0) || !isfinite(scale)) bad = true;
                         q[0] = Y[0] * scale; q[1] = Y[1] * scale; q[2] = Y[2] * scale;
                     }
@@ -466,7 +466,7 @@ int bdk_chain_step(bd_ctx* ctx, double* r, uint64_t first_step, int n_steps)
     ChainStepParams P;
     P.N = ctx->N; P.C = ctx->C;
     P.b = ctx->p.b; P.hstar = ctx->p.hstar; P.a_s = ctx->p.a / ctx->p.b; P.inv_a = ctx->p.b / ctx->p.a; P.inv_b = 1.0 / ctx->p.b;
-    P.K = ctx->p.K; P.dt = ctx->p.dt;
+    P.sl = make_spring_law(ctx->p); P.dt = ctx->p.dt;
     for (int i = 0; i < 9; ++i) P.kap[i] = ctx->p.kappa[i];
     P.seed = ctx->p.seed; P.chain0 = ctx->p.chain_id0; P.first_step = first_step;
     P.n_steps = n_steps; P.noise_kind = ctx->p.noise_kind;

@@ -10,7 +10,7 @@ namespace {
 
 constexpr int kObsThreads = 256;
 
-__global__ void __launch_bounds__(kObsThreads) k_obs_chain(int N, double K, double b, const double* __restrict__ r_all,
+__global__ void __launch_bounds__(kObsThreads) k_obs_chain(int N, SpringLaw sl, const double* __restrict__ r_all,
                                                            double* __restrict__ per_chain)
 {
     __shared__ double s_red[kObsThreads / 32][12];
@@ -42,7 +42,8 @@ __global__ void __launch_bounds__(kObsThreads) k_obs_chain(int N, double K, doub
         if (i < N) {
             const double qx = r[3 * i + 3] - r[3 * i], qy = r[3 * i + 4] - r[3 * i + 1], qz = r[3 * i + 5] - r[3 * i + 2];
             const double q = sqrt(qx * qx + qy * qy + qz * qz);
-            const double t = K * (q - b) / q;                     // Eq. 3: T = t Q
+            const double t = spring_coeff(sl, q);                 // Eq. 3 (or Eq. 4): T = t Q
+            const double b = sl.b;
             sxx += t * qx * qx; syy += t * qy * qy; szz += t * qz * qz;
             sxy += t * qx * qy; sxz += t * qx * qz; syz += t * qy * qz;
             const double dv = q - b;
@@ -163,7 +164,7 @@ int bdk_autocorr(bd_ctx* ctx, const double* r, const double* R0, double* out)
 int bdk_observables(bd_ctx* ctx, const double* r, double* per_chain, double* ensemble)
 {
     double* pc = (per_chain != nullptr) ? per_chain : ctx->obs;
-    BD_LAUNCH(ctx, k_obs_chain, dim3(ctx->C), dim3(kObsThreads), 0, ctx->N, ctx->p.K, ctx->p.b, r, pc);
+    BD_LAUNCH(ctx, k_obs_chain, dim3(ctx->C), dim3(kObsThreads), 0, ctx->N, make_spring_law(ctx->p), r, pc);
     if (ensemble != nullptr) BD_LAUNCH(ctx, k_obs_ensemble, dim3(1), dim3(BD_NOBS * 32), 0, ctx->C, pc, ensemble);
     return 0;
 }

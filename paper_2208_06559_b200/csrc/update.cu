@@ -64,15 +64,15 @@ __global__ void __launch_bounds__(kUpdThreads) k_init_walk(int N, double b, uint
 // -------------------------------------------------------------------------------------------------
 // a1: T_k = K (|Q_k| - b)/|Q_k| Q_k (Eq. 3, :76);  F_0 = T_0, F_j = T_j - T_{j-1}, F_N = -T_{N-1}
 // (Eq. 1 net spring term :68, Eq. 22 :235).  One thread per bead j computes T_{j-1} and T_j.
-__device__ __forceinline__ void tension(const double* __restrict__ r, int k, double K, double b, double T[3])
+__device__ __forceinline__ void tension(const double* __restrict__ r, int k, const SpringLaw& sl, double T[3])
 {
     const double qx = r[3 * k + 3] - r[3 * k], qy = r[3 * k + 4] - r[3 * k + 1], qz = r[3 * k + 5] - r[3 * k + 2];
     const double q = sqrt(qx * qx + qy * qy + qz * qz);
-    const double c = K * (q - b) / q;
+    const double c = spring_coeff(sl, q);
     T[0] = c * qx; T[1] = c * qy; T[2] = c * qz;
 }
 
-__global__ void __launch_bounds__(256) k_forces(int N, int nblk, double K, double b, const double* __restrict__ r_all,
+__global__ void __launch_bounds__(256) k_forces(int N, int nblk, SpringLaw sl, const double* __restrict__ r_all,
                                                 double* __restrict__ T_all, double* __restrict__ F_all)
 {
     const int c = blockIdx.x / nblk;                       // chain and block both on grid.x
@@ -80,8 +80,8 @@ __global__ void __launch_bounds__(256) k_forces(int N, int nblk, double K, doubl
     if (j > N) return;
     const double* r = r_all + (size_t)c * 3 * (N + 1);
     double Tl[3] = {0, 0, 0}, Tr[3] = {0, 0, 0};
-    if (j > 0) tension(r, j - 1, K, b, Tl);
-    if (j < N) tension(r, j, K, b, Tr);
+    if (j > 0) tension(r, j - 1, sl, Tl);
+    if (j < N) tension(r, j, sl, Tr);
     if (T_all != nullptr && j < N) {
         double* T = T_all + (size_t)c * 3 * N;
         T[3 * j] = Tr[0]; T[3 * j + 1] = Tr[1]; T[3 * j + 2] = Tr[2];
@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(256) k_drift(int N, int nblk, double hstar, do
 //         r'_0 = 0, r'_{k+1} = r'_k + Q'_k, centre of mass -> 0 (reading A8)
 // One CTA per chain.  A chain whose factorisation failed in THIS step (info_step != 0) or whose update is
 // non-finite keeps its positions for this step (reading A10); its first failure code is kept in info_sticky.
-struct UpdParams { double dt, K, b; double kap[9]; };
+struct UpdParams { double dt; SpringLaw sl; double kap[9]; };
 
 __global__ void __launch_bounds__(kUpdThreads) k_update(int N, UpdParams P, const double* __restrict__ r_all,
                                                         const double* __restrict__ v_all, const double* __restrict__ y_all,
@@ -149,14 +149,13 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(int N, UpdParams P, cons
     const int32_t code_in = (info_step != nullptr) ? info_step[c] : 0;       // this step's factorisation failure, if any
     const bool skip = code_in != 0;
     if (!skip) {
-        const double tdk = 2.0 * P.dt * P.K;
         rebuild_positions(N, tmp_all + c * M, r_out, s_buf, bad, [&](int k, double* q) {
             double ra[3], rb[3], Y[3];
 #pragma unroll
             for (int d = 0; d < 3; ++d) { ra[d] = r[3 * k + d]; rb[d] = r[3 * k + 3 + d]; }
             const double Qx = rb[0] - ra[0], Qy = rb[1] - ra[1], Qz = rb[2] - ra[2];
             const double qn = sqrt(Qx * Qx + Qy * Qy + Qz * Qz);
-            const double tc = P.K * (qn - P.b) / qn;                    // Eq. 3
+            const double tc = spring_coeff(P.sl, qn);                   // Eq. 3 (or Eq. 4)
             const double Q[3] = {Qx, Qy, Qz};
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
@@ -167,7 +166,7 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(int N, UpdParams P, cons
                 Y[d] = Q[d] + (ub - ua) + 2.0 * P.dt * (tc * Q[d]);
             }
             const double Yn = sqrt(Y[0] * Y[0] + Y[1] * Y[1] + Y[2] * Y[2]);
-            const double scale = ((tdk * P.b + Yn) / (tdk + 1.0)) / Yn;
+            const double scale = implicit_length(P.sl, Yn) / Yn;        // Eq. 17, then Eq. 15
             if (!(Yn > 0.0) || !isfinite(scale)) bad = true;
             q[0] = Y[0] * scale; q[1] = Y[1] * scale; q[2] = Y[2] * scale;
         });
@@ -194,7 +193,7 @@ int bdk_drift(bd_ctx* ctx, const double* r, double* T, double* F, double* v)
     double* Fbuf = (F != nullptr) ? F : ctx->F;
     if (T != nullptr || F != nullptr || v != nullptr)
         BD_LAUNCH(ctx, k_forces, dim3((unsigned)((int64_t)((ctx->Nb + 255) / 256) * ctx->C)), dim3(256), 0, ctx->N, (ctx->Nb + 255) / 256,
-                  ctx->p.K, ctx->p.b, r, T, Fbuf);
+                  make_spring_law(ctx->p), r, T, Fbuf);
     if (v != nullptr)
         BD_LAUNCH(ctx, k_drift, dim3((unsigned)((int64_t)((ctx->Nb + 7) / 8) * ctx->C)), dim3(256), 0, ctx->N, (ctx->Nb + 7) / 8, ctx->p.hstar,
                   ctx->p.a / ctx->p.b, ctx->p.b / ctx->p.a, 1.0 / ctx->p.b, r, Fbuf, v);
@@ -205,7 +204,7 @@ int bdk_update(bd_ctx* ctx, const double* r, const double* v, const double* y, c
                int32_t* info_sticky, double* r_out)
 {
     UpdParams P;
-    P.dt = ctx->p.dt; P.K = ctx->p.K; P.b = ctx->p.b;
+    P.dt = ctx->p.dt; P.sl = make_spring_law(ctx->p);
     for (int i = 0; i < 9; ++i) P.kap[i] = ctx->p.kappa[i];
     BD_LAUNCH(ctx, k_update, dim3(ctx->C), dim3(kUpdThreads), 0, ctx->N, P, r, v, y, info_step, info_sticky, ctx->tmp, r_out);
     return 0;

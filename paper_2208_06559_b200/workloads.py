@@ -94,3 +94,18 @@ def random_chains(n_chains: int, n_rods: int, b: float = 1.0, seed: int = 0,
     r[:, 1:, :] = np.cumsum(q, axis=1)
     r -= r.mean(axis=1, keepdims=True)
     return np.ascontiguousarray(r)
+
+
+def random_spring_chains(n_chains: int, n_springs: int, nu: float, b: float = 1.0, seed: int = 0,
+                         max_extension: float = 0.9) -> np.ndarray:
+    """Seeded bead-spring starts r[C][N_b][3] for the Cohen-Pade comparison model: Gaussian link
+    vectors with <Q^2> = nu b^2 (nu Kuhn steps per spring), clipped to max_extension of the full length nu b,
+    centre of mass at 0.  numpy Generator only; none of the method's arithmetic."""
+    rng = np.random.default_rng(seed)
+    q = rng.standard_normal((n_chains, n_springs, 3)) * math.sqrt(nu / 3.0) * b
+    length = np.linalg.norm(q, axis=-1, keepdims=True)
+    q *= np.minimum(1.0, max_extension * nu * b / length)
+    r = np.zeros((n_chains, n_springs + 1, 3), dtype=np.float64)
+    r[:, 1:, :] = np.cumsum(q, axis=1)
+    r -= r.mean(axis=1, keepdims=True)
+    return np.ascontiguousarray(r)

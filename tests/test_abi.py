@@ -33,7 +33,7 @@ def test_library_exports_every_declared_symbol():
 def test_binding_covers_every_declared_symbol():
     from paper_2208_06559_b200 import binding
     assert sorted(binding.EXPORTS) == _declared()
-    assert C.sizeof(binding.bd_params) == 4 + 4 + 8 * 5 + 8 * 9 + 8 + 8 + 8      # matches the C struct layout
+    assert C.sizeof(binding.bd_params) == 4 + 4 + 8 * 5 + 8 * 9 + 8 + 8 + 4 + 4 + 8      # matches the C struct layout
 
 
 def test_header_has_no_torch_or_cxx_types():
