@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(256, 2) k_trsm(double* __restrict__ A_all, int
 //   - C is loaded STRAIGHT INTO the accumulators (negated) when a tile starts and stored (negated back)
 //     when it ends: acc = -C + P P^T.  No load of C depends on anything in the epilogue, so the tensor
 //     pipe never waits on a DRAM round trip there (the first version's epilogue took 28 % of the
-//     kernel, profiles/r01_baseline_first_path.md); the next tile's C is prefetched into L2 meanwhile.
+//     kernel, profiles/r01_summary.md); the next tile's C is prefetched into L2 meanwhile.
 //   - the operand pipeline (cp.async ring of 128 x BK slabs, BK = 32, 2 stages) runs ACROSS tile boundaries: the
 //     load cursor is STAGES-1 k-slabs ahead of the compute cursor and simply moves on to the next tile.
 //   smem rows are padded to BK + 8 doubles: the 16-byte fragment loads (two k-steps each) are conflict free.

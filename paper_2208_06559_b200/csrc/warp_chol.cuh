@@ -5,7 +5,7 @@
 // Why: the diagonal-block factorisation is the serial part of every blocked Cholesky (M dependent pivots per
 // matrix).  Per pivot the dependency chain is
 //     SHFL (pivot broadcast) -> rsqrt (approx + one cubic correction + one Newton step) -> DMUL -> DFMA (next pivot)
-// ~ 130 cycles; everything else hangs off that chain.  Measured (profiles/r01_notes.md): a version that also
+// ~ 130 cycles; everything else hangs off that chain.  Measured (profiles/r01_summary.md): a version that also
 // carried the inverse in the same warp executed ~95 instructions per pivot at IPC 0.2 (566 cycles per pivot) --
 // the time went into issue slots, not into the chain -- so the inverse moved to its own warp.
 #pragma once

@@ -29,8 +29,12 @@ from .binding import BD, OBS_NAMES
 from .workloads import rouse_lambda
 
 
-def run(n_rods: int, n_chains: int, hstar: float, rate: float, dt: float, steps: int, samples: int, noise_kind: int):
-    kappa = np.diag([rate, -0.5 * rate, -0.5 * rate])
+def run(n_rods: int, n_chains: int, hstar: float, rate: float, dt: float, steps: int, samples: int, noise_kind: int,
+        flow: str = "extension"):
+    if flow == "shear":
+        kappa = np.zeros((3, 3)); kappa[0, 1] = rate                 # kappa_xy = shear rate
+    else:
+        kappa = np.diag([rate, -0.5 * rate, -0.5 * rate])
     bd = BD(n_rods=n_rods, n_chains=n_chains, dt=dt, hstar=hstar, kappa=kappa, seed=7, noise_kind=noise_kind)
     bd.set_workspace()
     r = bd.init_random_walk(2024)
@@ -45,7 +49,8 @@ def run(n_rods: int, n_chains: int, hstar: float, rate: float, dt: float, steps:
         p = per.cpu().numpy()
         n1 = p[:, i["Sxx"]] - p[:, i["Syy"]]
         rows.append((done * dt * rate, float(np.sqrt(p[:, i["R2"]].mean())), float(n1.mean()),
-                     float(n1.std(ddof=1) / np.sqrt(n_chains)), float(p[:, i["rod_dev_max"]].max())))
+                     float(n1.std(ddof=1) / np.sqrt(n_chains)), float(p[:, i["rod_dev_max"]].max()),
+                     float(np.sqrt(p[:, i["Ry2"]].mean()))))
         per_chain.append(np.sqrt(p[:, i["R2"]]))
         if done >= steps:
             break
@@ -72,29 +77,32 @@ def main():
     ap.add_argument("--hstar", type=float, nargs="+", default=[1e-5, 0.0, 0.5])
     ap.add_argument("--noise-kind", type=int, default=1, help="1 = the paper's uniform law (Eq. 2), 0 = Gaussian")
     ap.add_argument("--lam", choices=("rouse", "measured"), default="rouse")
+    ap.add_argument("--lam-value", type=float, default=0.0, help="use this relaxation time for every h* (e.g. the N^1.5 "
+                    "extrapolation of profiles/r02_relaxation.md for chains too long to measure)")
+    ap.add_argument("--flow", choices=("extension", "shear"), default="extension")
     args = ap.parse_args()
     lam_r = rouse_lambda(args.rods + 1)
-    print(f"BR-{args.rods}, {args.chains} chains, uniaxial extension Wi = {args.Wi}, dt = {args.dt}, K* = {1 / args.dt:g}, "
+    print(f"BR-{args.rods}, {args.chains} chains, start-up of {args.flow} Wi = {args.Wi}, dt = {args.dt}, K* = {1 / args.dt:g}, "
           f"noise kind {args.noise_kind}, to strain {args.strain}; lambda: {args.lam} (Rouse stand-in {lam_r:.4g})")
     res = {}
     for h in args.hstar:
-        lam = lam_r
-        if args.lam == "measured" and h >= 1e-3:
+        lam = args.lam_value if args.lam_value > 0 else lam_r
+        if args.lam_value <= 0 and args.lam == "measured" and h >= 1e-3:
             lam = relaxation.measure(args.rods, 2048, h, args.dt, 0.5, 200)["lambda"]
         rate = args.Wi / lam
         steps = int(round(args.strain / (rate * args.dt)))
-        rows, pc, ms, failed = run(args.rods, args.chains, h, rate, args.dt, steps, args.samples, args.noise_kind)
+        rows, pc, ms, failed = run(args.rods, args.chains, h, rate, args.dt, steps, args.samples, args.noise_kind, args.flow)
         res[h] = (rows, pc)
         print(f"h* = {h:g}: lambda {lam:.4g}, rate {rate:.4g}, {steps} steps in {ms / 1e3:.1f} s GPU time = {args.chains * steps / (ms * 1e-3):.4g} chain-steps/s, "
               f"{failed} failed chains, max ||Q|-b| = {max(r[4] for r in rows):.3g}", flush=True)
     hs = list(args.hstar)
-    print("\n| strain | " + " | ".join(f"R_ee (h* = {h:g}) | N_1 (h* = {h:g}) +- SE" for h in hs) + " |")
-    print("|---|" + "---|---|" * len(hs))
+    print("\n| strain | " + " | ".join(f"R_ee (h* = {h:g}) | sqrt<R_y^2> | N_1 (h* = {h:g}) +- SE" for h in hs) + " |")
+    print("|---|" + "---|---|---|" * len(hs))
     for k in range(len(res[hs[0]][0])):
         cells = []
         for h in hs:
-            s, ree, n1, se, _ = res[h][0][k]
-            cells.append(f"{ree:.4f} | {n1:.4g} +- {se:.2g}")
+            s, ree, n1, se, _, ry = res[h][0][k]
+            cells.append(f"{ree:.4f} | {ry:.4f} | {n1:.4g} +- {se:.2g}")
         print(f"| {res[hs[0]][0][k][0]:.3f} | " + " | ".join(cells) + " |")
     if len(hs) >= 2:
         a, b = res[hs[0]], res[hs[1]]
