@@ -85,9 +85,9 @@ __device__ __forceinline__ int warp_chol(double (&x)[NB], const int lane, double
 //     W[k][c] = (delta_kc - sum_{j<k} L[k][j] W[j][c]) / L[k][k]
 // L(k, j) (j < k) and s_rinv[k] come from shared memory as broadcast loads once the factoring warp has arrived on the
 // chunk's named barrier; rows k >= nrows (padding of a ragged block) are identity rows.  Row k goes to s_w[k*WS + c].
-template <int NB, int CH, int WS, class LoadL>
-__device__ __forceinline__ void warp_inverse(const int lane, const int nrows, const double* __restrict__ s_rinv,
-                                             double* __restrict__ s_w, const int bar0, LoadL&& L)
+template <int NB, int CH, class LoadL, class StoreW>
+__device__ __forceinline__ void warp_inverse_f(const int lane, const int nrows, const double* __restrict__ s_rinv, const int bar0,
+                                               LoadL&& L, StoreW&& store_w)
 {
     double w[NB];
 #pragma unroll
@@ -105,6 +105,16 @@ __device__ __forceinline__ void warp_inverse(const int lane, const int nrows, co
         } else {
             w[k] = s0;
         }
-        if (lane < NB) s_w[k * WS + lane] = w[k];
+        store_w(k, w[k]);                                   // W[k][lane]
     }
+}
+
+// the same with row k of W stored at s_w[k*WS + c]
+template <int NB, int CH, int WS, class LoadL>
+__device__ __forceinline__ void warp_inverse(const int lane, const int nrows, const double* __restrict__ s_rinv,
+                                             double* __restrict__ s_w, const int bar0, LoadL&& L)
+{
+    warp_inverse_f<NB, CH>(lane, nrows, s_rinv, bar0, L, [&](int k, double v) {
+        if (lane < NB) s_w[k * WS + lane] = v;
+    });
 }

@@ -5,7 +5,8 @@ PAPER.md:297-299: N = 199 .. 6399 rods, one chain per GPU, step time ~ N^1.2 for
 
 For every (C, N_b) it times `bd_step` (+ observables) with CUDA events, reports ms per ensemble step, chain-steps/s and
 the Cholesky stage in TFLOP/s, and fits the log-log slope of the step time.  `--context` adds bench-only comparator
-rows that are NOT part of libbd: `torch.linalg.cholesky` (cuSOLVER potrf / potrfBatched, "the paper's method on this
+rows that are NOT part of libbd: `torch.linalg.cholesky(D, out=preallocated)` (cuSOLVER potrf / potrfBatched through torch's
+wrapper: the call is out of place, so it includes torch's dispatch and one M^2 copy per chain; "the paper's method on this
 box") on the same matrices and an FP64 `torch.matmul` of 8192^3 (cuBLAS DGEMM).
 Prints a markdown table; synthetic seeded random-walk chains (workloads.py recipe), h* = a = 0.25, dt = 1e-4, no flow.
 """
@@ -60,7 +61,9 @@ def sweep(chains, beads, context=False):
                    "fused": stage["fused"] > 0, "failed": bd.last_info()[0]}
             if context and C * M * M * 8.0 < 20e9:        # comparator only where two extra copies of D fit comfortably
                 D = bd.assemble_hi(r)[:, :, :M].contiguous()
-                row["potrf_ms"] = _time(lambda: torch.linalg.cholesky(D), 3)
+                Lout = torch.empty_like(D)                    # preallocated result: no allocation inside the timed call
+                row["potrf_ms"] = _time(lambda: torch.linalg.cholesky(D, out=Lout), 3)
+                del Lout
                 row["potrf_tf"] = flops * C / (row["potrf_ms"] * 1e-3) / 1e12
                 del D
             rows.append(row)
@@ -89,7 +92,7 @@ def main():
     hdr = "| C | N_b | M | path | ms / ensemble step | chain-steps/s | Cholesky TFLOP/s |"
     sep = "|---|---|---|---|---|---|---|"
     if args.context:
-        hdr += " torch.linalg.cholesky ms (TFLOP/s) |"
+        hdr += " torch.linalg.cholesky(out=) ms (TFLOP/s): cuSOLVER potrf / potrfBatched through torch's wrapper |"
         sep += "---|"
     print(hdr)
     print(sep)
