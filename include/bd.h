@@ -42,6 +42,8 @@ extern "C" {
 #define BD_ERR_CUDA      (-100)   /* a CUDA runtime call failed; bd_strerror gives the text */
 #define BD_ERR_WORKSPACE (-101)   /* bd_step needs a workspace: call bd_set_workspace first  */
 #define BD_ERR_ALLOC     (-102)
+#define BD_ERR_INTERNAL  (-103)   /* bd_last_info: a dependency wait inside the tile Cholesky timed out (a bug, not a
+                                     numerical failure); results of that call are undefined                  */
 
 typedef struct bd_ctx bd_ctx;     /* opaque; one context per stream */
 

@@ -17,7 +17,7 @@ from . import build as _build
 NOBS = 13
 OBS_NAMES = ("R2", "Rx2", "Ry2", "Rz2", "Rg2", "Sxx", "Syy", "Szz", "Sxy", "Sxz", "Syz",
              "rod_dev_ms", "rod_dev_max")
-ERR_CUDA, ERR_WORKSPACE, ERR_ALLOC = -100, -101, -102
+ERR_CUDA, ERR_WORKSPACE, ERR_ALLOC, ERR_INTERNAL = -100, -101, -102, -103
 
 
 class bd_params(C.Structure):

@@ -318,8 +318,13 @@ int bd_last_info(bd_ctx* ctx, int32_t* n_failed_chains, int32_t* first_failed_ch
     int rc = bdk_count_failures(ctx, ctx->info);
     if (rc != 0) return rc;
     int32_t h[2] = {0, -1};
+    int32_t tile_err = 0;
     BD_CUDA(ctx, cudaMemcpyAsync(h, ctx->fail, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+    if (ctx->tile_flags != nullptr)                      // error word of the tile Cholesky (after its flags and ticket counter)
+        BD_CUDA(ctx, cudaMemcpyAsync(&tile_err, ctx->tile_flags + bdk_potrf_tiles_flag_words(ctx) + 1, sizeof(int32_t),
+                                     cudaMemcpyDeviceToHost, ctx->stream));
     BD_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (tile_err != 0) return BD_ERR_INTERNAL;
     if (n_failed_chains != nullptr) *n_failed_chains = h[0];
     if (first_failed_chain != nullptr) *first_failed_chain = h[1];
     return 0;
@@ -402,6 +407,7 @@ const char* bd_strerror(int code)
         case BD_ERR_CUDA: return (tl_create_cuda != cudaSuccess) ? cudaGetErrorString(tl_create_cuda) : "CUDA runtime error (bd_last_error(ctx) gives the text)";
         case BD_ERR_WORKSPACE: return "bd_step needs a workspace: call bd_set_workspace first";
         case BD_ERR_ALLOC: return "host allocation failed";
+        case BD_ERR_INTERNAL: return "internal error: a dependency wait inside the tile Cholesky timed out";
         default: break;
     }
     if (code < 0 && code > -20) return "invalid argument (index = -code)";

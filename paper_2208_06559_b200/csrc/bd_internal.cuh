@@ -76,6 +76,7 @@ int bdk_potrf(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
 int bdk_potrf_launches(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info);   // potrf.cu
 int bdk_potrf_tiles(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info);      // potrf_tiles.cu
 size_t bdk_potrf_tiles_scratch_bytes(const bd_ctx* ctx);
+size_t bdk_potrf_tiles_flag_words(const bd_ctx* ctx);      // ready flags [C][T][T]; then the ticket counter and the error word
 int bdk_noise(bd_ctx* ctx, uint64_t step, double* dW);
 int bdk_trmv(bd_ctx* ctx, const double* L, int64_t ld, int64_t stride, const double* dW, double* y);
 int bdk_drift(bd_ctx* ctx, const double* r, double* T, double* F, double* v);

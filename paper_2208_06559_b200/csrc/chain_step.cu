@@ -475,7 +475,8 @@ int bdk_chain_step(bd_ctx* ctx, double* r, uint64_t first_step, int n_steps)
     for (int i = 0; i < 9; ++i) P.kap[i] = ctx->p.kappa[i];
     P.seed = ctx->p.seed; P.chain0 = ctx->p.chain_id0; P.first_step = first_step;
     P.n_steps = n_steps; P.noise_kind = ctx->p.noise_kind;
-    P.r = r; P.scratch = ctx->ws; P.scratch_stride = (int64_t)MP * MP / 2 + 2 * (int64_t)MP;      // triangular fragment-major L of one chain P.info = ctx->info;
+    P.r = r; P.scratch = ctx->ws; P.info = ctx->info;
+    P.scratch_stride = (int64_t)MP * MP / 2 + 2 * (int64_t)MP;      // triangular fragment-major L of one chain
     int grid = ctx->num_sms * per_sm;
     if (grid > ctx->C) grid = ctx->C;
     BD_LAUNCH(ctx, k_chain_step<NT>, dim3(grid), dim3(CS_THREADS), smem, P);

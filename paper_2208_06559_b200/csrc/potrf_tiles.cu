@@ -48,7 +48,7 @@ constexpr long long SPIN_LIMIT = 8000000000LL;   // ~4 s of SM clocks: a lost de
 struct TileArgs {
     double* A;
     int64_t ld, stride;
-    int M, C, T;
+    int M, C, T, nsm;        // nsm = CTAs of the launch (one wave of tickets)
     double* Wbuf;            // [C][T][128][128] inverse diagonal blocks
     int* flags;              // [C][T][T]: == epoch when tile (i, j) of chain c is final
     int epoch;
@@ -77,13 +77,17 @@ __device__ __forceinline__ void wait_flag(const int* f, int epoch, int* err)
     }
 }
 
-// ticket -> (row i, column j, chain c).  Order: first the diagonal tile (0, 0) of every chain; then, for j = 0 .. T-2 and
-// inside it chain by chain, the tiles of column j with the NEXT diagonal tile slipped in early:
-//     (j+1, j), (j+1, j+1), (j+2, j), .., (T-1, j).
-// Tile (j+1, j+1) only needs row j+1 up to column j, so it can be factored while the rest of column j is still being
-// computed: when the tiles of column j+1 come up, L_{j+1,j+1} and its inverse have long been published.  Every tile
-// depends on tiles with smaller tickets only.
-__device__ __forceinline__ void decode_ticket(unsigned tk, int C, int T, int& j, int& c, int& i)
+// ticket -> (row i, column j, chain c).  Order: first the diagonal tile (0, 0) of every chain; then, for j = 0 .. T-2
+// ("phase j"), the tiles of column j chain by chain, with the NEXT diagonal tile (j+1, j+1) slipped in early: it only
+// needs row j+1 up to column j, so it is factored while the rest of column j is still being computed, and when the
+// tiles of column j+1 come up L_{j+1,j+1} and its inverse have long been published.
+//   one chain, or few:   (j+1, j), (j+1, j+1), (j+2, j), .., (T-1, j)                          per chain
+//   many chains:         the diagonal tile of chain c follows the column tiles of chain c + delta, delta chosen so that
+//                        about one wave of tickets (the grid size) lies between tile (j+1, j) and the diagonal tile that
+//                        reads it (otherwise the CTA that draws the diagonal tile waits ~20 us for its neighbour's
+//                        epilogue: 3 % of the c3 step); the last delta diagonal tiles close the phase.
+// Every tile depends on tiles with smaller tickets only.
+__device__ __forceinline__ void decode_ticket(unsigned tk, int C, int T, int nsm, int& j, int& c, int& i)
 {
     if (tk < (unsigned)C) { i = 0; j = 0; c = (int)tk; return; }
     const unsigned u = tk - (unsigned)C;
@@ -95,11 +99,32 @@ __device__ __forceinline__ void decode_ticket(unsigned tk, int C, int T, int& j,
     while (jj + 1 <= T - 2 && before(jj + 1) * C <= (long long)u) ++jj;
     while (jj > 0 && before(jj) * C > (long long)u) --jj;
     const long long rem = (long long)u - before(jj) * C;
-    const int w = T - jj;                                       // entries per chain in phase jj
-    c = (int)(rem / w);
-    const int idx = (int)(rem - (long long)c * w);
-    if (idx == 1) { i = jj + 1; j = jj + 1; }
-    else { i = jj + (idx == 0 ? 1 : idx); j = jj; }
+    const int w = T - jj;                                       // entries per chain in phase jj: w - 1 column tiles + 1 diagonal tile
+    const int delta = min(C / 2, (nsm + 12 + w - 1) / w);
+    j = jj;
+    if (delta == 0) {
+        c = (int)(rem / w);
+        const int idx = (int)(rem - (long long)c * w);
+        if (idx == 1) { i = jj + 1; j = jj + 1; }
+        else i = jj + (idx == 0 ? 1 : idx);
+        return;
+    }
+    const int cw = w - 1;
+    if (rem < (long long)delta * cw) {                          // the first delta chains: column tiles only
+        c = (int)(rem / cw);
+        i = jj + 1 + (int)(rem - (long long)c * cw);
+        return;
+    }
+    const long long r2 = rem - (long long)delta * cw;
+    if (r2 < (long long)(C - delta) * w) {                      // column tiles of chain delta + g, then the diagonal tile of chain g
+        const int gq = (int)(r2 / w), idx = (int)(r2 - (long long)gq * w);
+        if (idx < cw) { c = delta + gq; i = jj + 1 + idx; }
+        else { c = gq; i = jj + 1; j = jj + 1; }
+        return;
+    }
+    c = C - delta + (int)(r2 - (long long)(C - delta) * w);     // the remaining diagonal tiles
+    i = jj + 1;
+    j = jj + 1;
 }
 
 // One 128 x 16 box of both operands: 2 chunk pairs x (4 + (8 - NTLO) LDS.128, 2 x 4 x (8 - NTLO) DMMA) per warp.  NTLO > 0 skips
@@ -193,7 +218,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_potrf_tiles(const __grid_consta
             mbar_arrive(bar_qf + 8 * qs);              // release: the consumers read sQ after their wait
             if (tk >= a.total) break;
             int i, j, c;
-            decode_ticket(tk, a.C, T, j, c, i);
+            decode_ticket(tk, a.C, T, a.nsm, j, c, i);
             const bool diag = (i == j);
             const int KT = j * SPB;                    // ring stages of the K loop
             int* flags_c = a.flags + (size_t)c * T * T;
@@ -273,7 +298,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_potrf_tiles(const __grid_consta
         if (lane == 0) mbar_arrive(bar_qe + 8 * qs);
         if (tk >= a.total) break;
         int i, j, c;
-        decode_ticket(tk, a.C, T, j, c, i);
+        decode_ticket(tk, a.C, T, a.nsm, j, c, i);
         const bool diag = (i == j);
         const int KT = j * SPB;
         double* A = a.A + (size_t)c * a.stride;
@@ -449,6 +474,12 @@ size_t bdk_potrf_tiles_scratch_bytes(const bd_ctx* ctx)
     return sizeof(double) * (size_t)ctx->C * T * TB * TB;
 }
 
+size_t bdk_potrf_tiles_flag_words(const bd_ctx* ctx)
+{
+    const size_t T = (size_t)(ctx->M + TB - 1) / TB;
+    return (size_t)ctx->C * T * T;
+}
+
 int bdk_potrf_tiles(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t* info)
 {
     const int M = ctx->M, C = ctx->C, T = (M + TB - 1) / TB;
@@ -484,7 +515,7 @@ int bdk_potrf_tiles(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t*
         ctx->tile_mapA_ptr = A; ctx->tile_mapA_ld = ld; ctx->tile_mapA_stride = stride;
     }
     TileArgs a;
-    a.A = A; a.ld = ld; a.stride = stride; a.M = M; a.C = C; a.T = T;
+    a.A = A; a.ld = ld; a.stride = stride; a.M = M; a.C = C; a.T = T; a.nsm = ctx->num_sms;
     a.Wbuf = ctx->tile_W;
     a.flags = ctx->tile_flags;
     a.epoch = ++ctx->tile_epoch;
