@@ -9,7 +9,7 @@ CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libbd.so")
 SOURCES = ["api.cu", "assemble.cu", "potrf.cu", "potrf_tiles.cu", "brownian.cu", "update.cu", "observables.cu", "chain_step.cu"]
-HEADERS = ["bd_internal.cuh", "philox.cuh", "block_ops.cuh", "warp_chol.cuh", "potf2_blocked.cuh", "tma.cuh", "dtile.cuh"]
+HEADERS = ["bd_internal.cuh", "philox.cuh", "block_ops.cuh", "warp_chol.cuh", "potf2_blocked.cuh", "tma.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr", "--extended-lambda"]
 

@@ -89,10 +89,9 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
     auto TIDX = [&](int r, int c) { return (c >> 2) * MT4 + r * 4 + (c & 3); };
 
     double* Lg = P.scratch + (size_t)blockIdx.x * P.scratch_stride;
-    // TRIANGULAR fragment-major storage: k-group q (columns 4q .. 4q+3) keeps rows 4q .. MP-1 only (nothing above the
-    // diagonal is ever read), MP^2/2 + 2 MP doubles per chain slot instead of MP^2: the scratch of all resident CTAs then
-    // fits in L2 (c2: 296 x 0.37 MB = 110 MB; the square layout spilled 356 MB per launch to DRAM).
-    auto lg_off = [&](int q) { return (size_t)4 * ((size_t)q * MP - (size_t)2 * q * (q - 1)); };   // doubles before k-group q
+    // (A triangular Lg -- rows >= 4 (col / 4) only, 110 MB instead of 219 MB for the 296 resident CTAs of c2, all of it in
+    // L2 -- was measured in round 2: 6 % SLOWER (9.77e5 against 1.04e6 chain-steps/s): the offset arithmetic costs more than
+    // the DRAM spill, which is not the limiter at 0.37 TB/s.)
     const uint32_t bar_full = smem_u32(&sBar[0]), bar_empty = smem_u32(&sBar[CS_STAGES]);
     const uint32_t ring_u32 = smem_u32(ring);
     if (tid == 0) {
@@ -153,7 +152,7 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                     if (Gs >= CS_STAGES) mbar_wait(bar_empty + 8 * sl, ((Gs / CS_STAGES) - 1) & 1);
                     mbar_expect_tx(bar_full + 8 * sl, kg * stage_bytes);
                     for (int h = 0; h < kg; ++h)
-                        tma_bulk_g2s(ring_u32 + (sl * slot_s + h * sub_d) * 8, Lg + lg_off(qs * kg + h) + (size_t)(k0 - 4 * (qs * kg + h)) * 4, stage_bytes,
+                        tma_bulk_g2s(ring_u32 + (sl * slot_s + h * sub_d) * 8, Lg + ((size_t)(qs * kg + h) * MP + k0) * 4, stage_bytes,
                                      bar_full + 8 * sl);
                 };
                 if (tid == 0) {
@@ -371,8 +370,7 @@ __global__ void __launch_bounds__(CS_THREADS, (NT <= 3) ? 2 : 1) k_chain_step(Ch
                         // NEXT CTA's scratch (rows 8mt.. of its k-groups 0, 1) and corrupt a chain in flight there
                         if (k0 + 8 * nt >= MP) continue;
                         const int q = (k0 >> 2) + 2 * nt + (t >> 1);
-                        if (8 * mt + g < 4 * q) continue;                // above the diagonal of L_kk: not stored (triangular layout)
-                        *reinterpret_cast<double2*>(Lg + lg_off(q) + (size_t)(8 * mt + g - 4 * q) * 4 + 2 * (t & 1)) = make_double2(x[nt][0], x[nt][1]);
+                        *reinterpret_cast<double2*>(Lg + ((size_t)q * MP + 8 * mt + g) * 4 + 2 * (t & 1)) = make_double2(x[nt][0], x[nt][1]);
                     }
                     part += __shfl_xor_sync(0xffffffffu, part, 1);
                     part += __shfl_xor_sync(0xffffffffu, part, 2);
@@ -476,7 +474,7 @@ int bdk_chain_step(bd_ctx* ctx, double* r, uint64_t first_step, int n_steps)
     P.seed = ctx->p.seed; P.chain0 = ctx->p.chain_id0; P.first_step = first_step;
     P.n_steps = n_steps; P.noise_kind = ctx->p.noise_kind;
     P.r = r; P.scratch = ctx->ws; P.info = ctx->info;
-    P.scratch_stride = (int64_t)MP * MP / 2 + 2 * (int64_t)MP;      // triangular fragment-major L of one chain
+    P.scratch_stride = (int64_t)MP * MP;
     int grid = ctx->num_sms * per_sm;
     if (grid > ctx->C) grid = ctx->C;
     BD_LAUNCH(ctx, k_chain_step<NT>, dim3(grid), dim3(CS_THREADS), smem, P);

@@ -6,7 +6,7 @@
 //     acc = -D_ij + sum_{k < 128 j} L[i-rows][k] L[j-rows][k]       K-deep FP64 tensor-core (DMMA m8n8k4) loop, the
 //                                                                    C tile never leaves the accumulators
 //     i > j:  S = -acc;  L_ij = S W_j^T  with W_j = L_jj^-1          a second, 128-deep pass through the same pipeline
-//     i = j:  L_jj = chol(S), W_j = L_jj^-1                          in shared memory (dtile.cuh: 16-column panels)
+//     i = j:  L_jj = chol(S), W_j = L_jj^-1                          in shared memory (potf2_blocked.cuh, 64 + 64)
 //   Tickets are handed out column by column (j outer, then chain, then i, the next diagonal tile early); a tile waits (ld.acquire on the ready flag
 //   of the tiles it reads) only for tiles with SMALLER tickets, which running CTAs own, so the schedule cannot
 //   deadlock and needs no co-residency.  Later columns start while the diagonal block of the current one is still being
@@ -25,7 +25,7 @@
 #include <cuda.h>          // CUtensorMap and its enums only; cuTensorMapEncodeTiled is fetched through the runtime (no -lcuda)
 
 #include "bd_internal.cuh"
-#include "dtile.cuh"
+#include "potf2_blocked.cuh"
 #include "tma.cuh"
 
 namespace {
@@ -405,13 +405,17 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_potrf_tiles(const __grid_consta
             cons_sync();
             if (tid == 0) st_release_gpu(flags_c + (size_t)i * T + j, a.epoch);
         } else {
-            // ---- diagonal tile: S -> shared memory, L_jj = chol(S) and W_j = L_jj^-1 (dtile.cuh) -----------------
+            // ---- diagonal tile: S -> shared memory, L_jj = chol(S) and W_j = L_jj^-1 as 64 + 64 -------------
             cons_sync();                                          // every warp is done with the ring
-            double* X = reinterpret_cast<double*>(ring_g);        // [128][129]: L lower, W^T strict upper
-            double* Tb = X + dtile::N * dtile::LDX;               // [64][65] scratch of the inverse
-            double* rinv = Tb + 64 * dtile::LDT;                  // [128] 1 / L_ii
-            double* sCol = rinv + dtile::N;                       // [64] column buffer of warp_chol
+            double* S11 = reinterpret_cast<double*>(ring_g);
+            double* S21 = S11 + 64 * potf2::SLDP;
+            double* S22 = S21 + 64 * potf2::SLDP;
+            double* W11 = S22 + 64 * potf2::SLDP;
+            double* W22 = W11 + 64 * potf2::SLDP;
+            double* sCol = W22 + 64 * potf2::SLDP;
+            double* sRinv = sCol + 64;
             const int nloc = min(TB, M - tn0);                    // rows / columns of the block that exist
+            for (int idx = tid; idx < 64 * potf2::SLDP; idx += NCONS) { W11[idx] = 0.0; W22[idx] = 0.0; }
             if (warp_active) {
 #pragma unroll
                 for (int mt = 0; mt < 4; ++mt) {
@@ -421,22 +425,81 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_potrf_tiles(const __grid_consta
 #pragma unroll
                         for (int e = 0; e < 2; ++e) {
                             const int Cc = wn * 64 + nt * 8 + 2 * t + e;
-                            if (Cc > R) continue;
-                            double v = -acc[mt][nt][e];
+                            double v = (Cc <= R) ? -acc[mt][nt][e] : 0.0;
                             if (R >= nloc || Cc >= nloc) v = (R == Cc) ? 1.0 : 0.0;       // identity padding (ragged tile)
-                            X[R * dtile::LDX + Cc] = v;
+                            double* dst = (R < 64) ? S11 + R * potf2::SLDP + Cc
+                                                   : (Cc < 64 ? S21 + (R - 64) * potf2::SLDP + Cc : S22 + (R - 64) * potf2::SLDP + (Cc - 64));
+                            if (R >= 64 || Cc < 64) *dst = v;
                         }
                 }
             }
             if (tid == 0) sFail = 0;
             cons_sync();
-            dtile::factor_invert(X, Tb, rinv, sCol, lane, warp, tn0, &sFail, [] { cons_sync(); });
-            // L -> the matrix (lower triangle only), W (full square, zeros above the diagonal) -> Wbuf
+            const int g64r = 16 * (warp & 3), g64c = 32 * (warp >> 2);     // gemm64 output block of this warp
+            double o[2][4][2];
+#pragma unroll 1
+            for (int hh = 0; hh < 2; ++hh) {
+                double* Sb = hh ? S22 : S11;
+                double* Wb = hh ? W22 : W11;
+                const int nrem = nloc - 64 * hh;
+                potf2::block64(Sb, Wb, sCol, sRinv, (nrem > potf2::HB) ? 2 : 1, lane, warp, tn0 + 64 * hh, &sFail, [] { cons_sync(); });
+                if (hh == 0) {
+                    potf2::gemm64(S21, W11, false, warp, lane, o);             // L21 = S21 W11^T
+                    cons_sync();
+#pragma unroll
+                    for (int mm = 0; mm < 2; ++mm)
+#pragma unroll
+                        for (int nn = 0; nn < 4; ++nn) {
+                            const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t;
+                            S21[r * potf2::SLDP + cc] = o[mm][nn][0];
+                            S21[r * potf2::SLDP + cc + 1] = o[mm][nn][1];
+                            const int gi = tn0 + 64 + r;
+                            if (gi < M) *reinterpret_cast<double2*>(A + (size_t)gi * ld + tn0 + cc) = make_double2(o[mm][nn][0], o[mm][nn][1]);
+                        }
+                    cons_sync();
+                    potf2::gemm64(S21, S21, false, warp, lane, o);             // S22 -= L21 L21^T (lower part)
+#pragma unroll
+                    for (int mm = 0; mm < 2; ++mm)
+#pragma unroll
+                        for (int nn = 0; nn < 4; ++nn)
+#pragma unroll
+                            for (int e = 0; e < 2; ++e) {
+                                const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t + e;
+                                if (cc <= r && 64 + r < nloc) S22[r * potf2::SLDP + cc] -= o[mm][nn][e];
+                            }
+                    cons_sync();
+                }
+            }
+            potf2::gemm64(S21, W11, true, warp, lane, o);                      // Tm = L21 W11
+            cons_sync();
+#pragma unroll
+            for (int mm = 0; mm < 2; ++mm)
+#pragma unroll
+                for (int nn = 0; nn < 4; ++nn) {
+                    const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t;
+                    S21[r * potf2::SLDP + cc] = o[mm][nn][0];
+                    S21[r * potf2::SLDP + cc + 1] = o[mm][nn][1];
+                }
+            cons_sync();
+            potf2::gemm64(W22, S21, true, warp, lane, o);                      // W21 = -W22 Tm
             double* Wg = a.Wbuf + ((size_t)c * T + j) * TB * TB;
-            for (int idx = tid; idx < TB * TB; idx += NCONS) {
-                const int r = idx >> 7, cc = idx & (TB - 1);
-                if (cc <= r && tn0 + r < M) A[(size_t)(tn0 + r) * ld + tn0 + cc] = X[r * dtile::LDX + cc];
-                Wg[idx] = dtile::w_el(X, rinv, r, cc);
+#pragma unroll
+            for (int mm = 0; mm < 2; ++mm)
+#pragma unroll
+                for (int nn = 0; nn < 4; ++nn) {
+                    const int r = g64r + 8 * mm + g, cc = g64c + 8 * nn + 2 * t;
+                    *reinterpret_cast<double2*>(Wg + (size_t)(64 + r) * TB + cc) = make_double2(-o[mm][nn][0], -o[mm][nn][1]);
+                }
+            // L11, L22 -> the matrix (lower triangle only); W11, 0, W22 -> Wbuf
+            for (int idx = tid; idx < 64 * 64; idx += NCONS) {
+                const int r = idx >> 6, cc = idx & 63;
+                if (cc <= r) {
+                    if (tn0 + r < M) A[(size_t)(tn0 + r) * ld + tn0 + cc] = S11[r * potf2::SLDP + cc];
+                    if (tn0 + 64 + r < M) A[(size_t)(tn0 + 64 + r) * ld + tn0 + 64 + cc] = S22[r * potf2::SLDP + cc];
+                }
+                Wg[(size_t)r * TB + cc] = W11[r * potf2::SLDP + cc];
+                Wg[(size_t)r * TB + 64 + cc] = 0.0;
+                Wg[(size_t)(64 + r) * TB + 64 + cc] = W22[r * potf2::SLDP + cc];
             }
             __threadfence();
             fence_proxy_async();
