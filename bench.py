@@ -285,7 +285,7 @@ def measure_config(w, K, warmup, rank, local_rank, world, path, sampler, peak_tf
     traffic, traffic_source = _traffic(w.name)
     roofline = {"bound": "tensor",
                 "kernel": "k_chain_step<3> (fused a0-a8, one launch per step)" if fused else
-                          "bd_cholesky stage of bd_step (FP64 DMMA: k_potf2 + k_trsm + k_syrk)",
+                          "bd_cholesky stage of bd_step = ONE launch of k_potrf_tiles (persistent tile Cholesky: TMA operands, FP64 DMMA)",
                 "achieved": chol_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": (chol_tflops / peak_tflops) if (chol_tflops and peak_tflops) else None,
                 "frac_datasheet_40": (chol_tflops / 40.0) if chol_tflops else None,

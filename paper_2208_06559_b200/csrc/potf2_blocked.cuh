@@ -18,7 +18,8 @@
 namespace potf2 {
 
 constexpr int HB = 32;            // half block
-constexpr int SLDP = 65;          // row stride of the 64 x 64 working copies (odd: conflict-free columns)
+constexpr int SLDP = 68;          // row stride of the 64 x 64 working copies: (4 g + t) mod 16 is distinct over a half-warp, so the 8-byte DMMA fragment loads
+                                  // of the products are conflict free (65 gave up to 4-way conflicts there; the column accesses of the factoring warp are 4-way now, once per pivot)
 
 // out = sum_p X[i][p] * Y(j, p): product of two 32 x 32 operands held in shared memory on the FP64 tensor cores.
 // Warp w owns output rows 8 (w & 3) .. +7 and columns 16 (w >> 2) .. +15 (two m8n8k4 accumulators, 8 k-steps);
@@ -72,13 +73,20 @@ __device__ __forceinline__ void gemm64(const double* __restrict__ X, const doubl
     }
 }
 
-// rows / columns o .. o+31 of the working copy: warp 0 factors (L back into S, 1 / L_kk into s_rinv), warp 1 forms the
-// inverse of that 32 x 32 factor in Wm, 4 pivots behind (named barriers 1..8).  Called from ONE place (a loop over the two
-// halves): the fully unrolled pivot loops are ~1700 straight-line instructions, and a second inlined copy ran 4x slower.
+// rows / columns o .. o+31 of the working copy: warp 0 factors (L back into S, 1 / L_kk into s_rinv); the inverse of that
+// 32 x 32 factor is formed in Wm as 16 + 16 so that it ends right behind the factorisation instead of 7 k cycles later
+// (a single warp inverting all 32 rows by substitution is slower than the factoring warp: 17.5 k against 10 k cycles,
+// profiles/r02_summary.md):
+//     warp 1   W11 = L11^-1   rows 0..15,  4 pivots behind the factoring warp           (named barriers 1..4)
+//     warp 2   W22 = L22^-1   rows 16..31, 4 pivots behind                              (named barriers 5..8)
+//              then W21 = -W22 (L21 W11): two 16 x 16 x 16 products on the tensor cores (named barrier 10: W11 is ready)
+// Called from ONE place (a loop over the two halves): the fully unrolled pivot loops are ~1700 straight-line
+// instructions, and a second inlined copy ran 4x slower.
 __device__ __forceinline__ void factor_half(double* __restrict__ S, double* __restrict__ Wm, double* __restrict__ sCol,
                                             double* __restrict__ sRinv, const int o, const int lane, const int warp, const int j0,
                                             int* sFail)
 {
+    constexpr int QB = HB / 2;
     if (warp == 0) {
         double x[HB];
 #pragma unroll
@@ -89,7 +97,52 @@ __device__ __forceinline__ void factor_half(double* __restrict__ S, double* __re
         });
         if (lane == 0 && f != 0 && *sFail == 0) *sFail = j0 + o + f;
     } else if (warp == 1) {
-        warp_inverse<HB, 4, SLDP>(lane, HB, sRinv + o, Wm + o * SLDP + o, 1, [&](int k, int j) { return S[(o + k) * SLDP + o + j]; });
+        warp_inverse_f<QB, 4>(lane, QB, sRinv + o, 1, [&](int k, int j) { return S[(o + k) * SLDP + o + j]; },
+                              [&](int k, double v) {
+                                  if (lane < QB) Wm[(o + k) * SLDP + o + lane] = v;
+                              });
+        named_arrive(10, 64);
+    } else if (warp == 2) {
+        const int o2 = o + QB;
+        warp_inverse_f<QB, 4>(lane, QB, sRinv + o2, 1 + QB / 4, [&](int k, int j) { return S[(o2 + k) * SLDP + o2 + j]; },
+                              [&](int k, double v) {
+                                  if (lane < QB) Wm[(o2 + k) * SLDP + o2 + lane] = v;
+                              });
+        named_sync(10, 64);
+        // T = L21 W11 (into the W21 area), then W21 = -W22 T; lane (g, t) holds elements (8 mt + g, 8 nt + 2 t + {0, 1})
+        const int g = lane >> 2, t = lane & 3;
+        double o4[2][2][2];
+#pragma unroll
+        for (int pass = 0; pass < 2; ++pass) {
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < 2; ++nt) {
+                    double c0 = 0.0, c1 = 0.0;
+#pragma unroll
+                    for (int ks = 0; ks < QB / 4; ++ks) {
+                        const int i = 8 * mt + g, k = 4 * ks + t, j = 8 * nt + g;
+                        // pass 0: A = L21 (S), B = W11;  pass 1: A = W22, B = T (both in Wm)
+                        const double av = pass ? Wm[(o2 + i) * SLDP + o2 + k] : S[(o2 + i) * SLDP + o + k];
+                        const double bv = pass ? Wm[(o2 + k) * SLDP + o + j] : Wm[(o + k) * SLDP + o + j];
+                        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                                     : "+d"(c0), "+d"(c1)
+                                     : "d"(av), "d"(bv));
+                    }
+                    o4[mt][nt][0] = c0;
+                    o4[mt][nt][1] = c1;
+                }
+            __syncwarp();
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < 2; ++nt) {
+                    double* dst = Wm + (o2 + 8 * mt + g) * SLDP + o + 8 * nt + 2 * t;
+                    dst[0] = pass ? -o4[mt][nt][0] : o4[mt][nt][0];
+                    dst[1] = pass ? -o4[mt][nt][1] : o4[mt][nt][1];
+                }
+            __syncwarp();
+        }
     }
 }
 
