@@ -103,3 +103,35 @@ def test_staged_step_with_either_cholesky(algo):
     ro, info = O.step_ensemble(O.Params(n_rods=N, dt=dt, kappa=kap, seed=4), r0, 0, 1)
     assert not info.any() and bd.last_info() == (0, -1)
     assert np.abs(rg - ro).max() / np.abs(ro).max() <= 1e-10
+
+
+def test_two_contexts_on_two_streams_factor_concurrently():
+    """every context owns its flags, ticket counter and inverse blocks, and a tile only waits for tiles with smaller
+    tickets of its OWN launch: two persistent tile kernels in flight on two streams finish and agree with the oracle."""
+    from paper_2208_06559_b200.binding import BD
+    N, C = 300, 2
+    r = W.random_chains(2 * C, N, seed=77, rod_jitter=0.01)
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    bds, Ds = [], []
+    for k, st in enumerate(streams):
+        with torch.cuda.stream(st):
+            bd = BD(n_rods=N, n_chains=C, dt=1e-4, stream=st)
+            bd.set_cholesky(2)
+            D = bd.matrix_storage()
+            bd.assemble_hi(_dev(r[k * C:(k + 1) * C]), D)
+            bds.append(bd); Ds.append(D)
+    torch.cuda.synchronize()
+    for rep in range(3):                                  # launches interleave on the two streams
+        for bd, D, st in zip(bds, Ds, streams):
+            with torch.cuda.stream(st):
+                if rep:
+                    bd.assemble_hi(_dev(r[bds.index(bd) * C:(bds.index(bd) + 1) * C]), D)
+                bd.cholesky(D)
+    torch.cuda.synchronize()
+    p = O.Params(n_rods=N, dt=1e-4)
+    for k, (bd, D) in enumerate(zip(bds, Ds)):
+        assert bd.last_info() == (0, -1)
+        Lh = _host(D)
+        for c in range(C):
+            Lo, io = O.cholesky(O.assemble(p, r[k * C + c]))
+            assert io == 0 and np.linalg.norm(np.tril(Lh[c, :, :bd.M]) - Lo) <= 1e-12 * np.linalg.norm(Lo)
