@@ -548,11 +548,14 @@ int bdk_potrf_tiles(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t*
     const int M = ctx->M, C = ctx->C, T = (M + TB - 1) / TB;
     const uint64_t total64 = (uint64_t)C * T * (T + 1) / 2;
     if (total64 + 1024 > 0xffffffffull || (uint64_t)C * T * TB > 0x7fffffffull) return BD_ERR_ALLOC;
-    if (ctx->tile_W == nullptr) {
-        BD_CUDA(ctx, cudaMalloc(&ctx->tile_W, bdk_potrf_tiles_scratch_bytes(ctx)));
+    if (ctx->tile_flags == nullptr) {                 // first factorisation of this context (flags are allocated last)
+        if (ctx->tile_W == nullptr) BD_CUDA(ctx, cudaMalloc(&ctx->tile_W, bdk_potrf_tiles_scratch_bytes(ctx)));
         const size_t fb = sizeof(int) * ((size_t)C * T * T + 2);
-        BD_CUDA(ctx, cudaMalloc(&ctx->tile_flags, fb));
-        BD_CUDA(ctx, cudaMemsetAsync(ctx->tile_flags, 0, fb, ctx->stream));
+        int* flags = nullptr;
+        BD_CUDA(ctx, cudaMalloc(&flags, fb));
+        cudaError_t e0 = cudaMemsetAsync(flags, 0, fb, ctx->stream);
+        if (e0 != cudaSuccess) { cudaFree(flags); ctx->last_cuda = e0; return BD_ERR_CUDA; }
+        ctx->tile_flags = flags;
         ctx->tile_epoch = 0;
         ctx->tile_ticket_base = 0;
         BD_CUDA(ctx, cudaFuncSetAttribute(k_potrf_tiles, cudaFuncAttributeMaxDynamicSharedMemorySize, TILE_SMEM));
