@@ -42,6 +42,7 @@ extern "C" {
 #define BD_ERR_CUDA      (-100)   /* a CUDA runtime call failed; bd_strerror gives the text */
 #define BD_ERR_WORKSPACE (-101)   /* bd_step needs a workspace: call bd_set_workspace first  */
 #define BD_ERR_ALLOC     (-102)
+#define BD_ERR_TOO_LARGE (-104)   /* bd_cholesky_noalloc: problem beyond its fixed scratch (see there)           */
 #define BD_ERR_INTERNAL  (-103)   /* bd_last_info: a dependency wait inside the tile Cholesky timed out (a bug, not a
                                      numerical failure); results of that call are undefined                  */
 
@@ -102,6 +103,22 @@ int bd_cholesky(bd_ctx *ctx, double *DL_dev, int64_t ld, int64_t chain_stride, i
  * dW is read from dW_dev_or_null [C][M].                                                         */
 int bd_brownian(bd_ctx *ctx, const double *L_dev, int64_t ld, int64_t chain_stride, uint64_t step,
                 const double *dW_dev_or_null, double *y_dev);
+
+/* a3 WITHOUT ANY ALLOCATION, for callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops,
+ * harnesses that forbid it): the same tile Cholesky as bd_cholesky, with its scratch (inverse diagonal blocks, ready
+ * flags, ticket counter) in a fixed file-scope device array of 4 MB + 4.2 KB that every GPU that loads the library
+ * holds until exit.  No context: DL_dev [n_chains] matrices of order M, layout as for bd_cholesky (row-major, ld >= M
+ * even, chain_stride >= ld*M even, base 16-byte aligned, lower triangle in and out); info_dev [n_chains] int32 or NULL
+ * (cleared, then 1-based failing pivot row per chain); cuda_stream a cudaStream_t (NULL = default stream); the device
+ * current at the call is used.  Asynchronous on that stream.  The call itself issues no cudaMalloc / cudaFree; its first
+ * call on a device looks up the array's address (cudaGetSymbolAddress).
+ * LIMIT: n_chains * ceil(M / 128) <= 32 (one chain of M <= 4096, 2 of M <= 2048, 8 of M <= 512, 32 of M <= 128);
+ * beyond it BD_ERR_TOO_LARGE and nothing is launched.  Returns -k for the k-th invalid argument.
+ * ALL calls share the one array: calls that overlap on the GPU (different streams or host threads) race and give
+ * undefined results -- serialise them.  It keeps the last call's contents; what must start at zero is cleared on the
+ * stream at the start of each call.                                                                              */
+int bd_cholesky_noalloc(double *DL_dev, int32_t M, int32_t n_chains, int64_t ld, int64_t chain_stride,
+                        int32_t *info_dev, void *cuda_stream);
 
 /* The Brownian increments alone: dW_dev [C][M] for time step `step`.                             */
 int bd_noise(bd_ctx *ctx, uint64_t step, double *dW_dev);

@@ -17,7 +17,7 @@ from . import build as _build
 NOBS = 13
 OBS_NAMES = ("R2", "Rx2", "Ry2", "Rz2", "Rg2", "Sxx", "Syy", "Szz", "Sxy", "Sxz", "Syz",
              "rod_dev_ms", "rod_dev_max")
-ERR_CUDA, ERR_WORKSPACE, ERR_ALLOC, ERR_INTERNAL = -100, -101, -102, -103
+ERR_CUDA, ERR_WORKSPACE, ERR_ALLOC, ERR_INTERNAL, ERR_TOO_LARGE = -100, -101, -102, -103, -104
 
 
 class bd_params(C.Structure):
@@ -28,7 +28,7 @@ class bd_params(C.Structure):
 
 
 EXPORTS = ("bd_create", "bd_destroy", "bd_workspace_bytes", "bd_set_workspace", "bd_set_flow",
-           "bd_init_random_walk", "bd_assemble_hi", "bd_cholesky", "bd_brownian", "bd_noise", "bd_drift",
+           "bd_init_random_walk", "bd_assemble_hi", "bd_cholesky", "bd_cholesky_noalloc", "bd_brownian", "bd_noise", "bd_drift",
            "bd_update", "bd_set_path", "bd_set_cholesky", "bd_step", "bd_observables", "bd_end_to_end", "bd_autocorr", "bd_last_info", "bd_step_host", "bd_profile",
            "bd_stage_ms", "bd_launch_count", "bd_strerror", "bd_last_error")
 
@@ -54,6 +54,7 @@ def load_library(path: str | None = None) -> C.CDLL:
     lib.bd_init_random_walk.argtypes = [vp, dp, u64]
     lib.bd_assemble_hi.argtypes = [vp, dp, dp, i64, i64, i32]
     lib.bd_cholesky.argtypes = [vp, dp, i64, i64, dp]
+    lib.bd_cholesky_noalloc.argtypes = [dp, i32, i32, i64, i64, dp, vp]
     lib.bd_brownian.argtypes = [vp, dp, i64, i64, u64, dp, dp]
     lib.bd_noise.argtypes = [vp, u64, dp]
     lib.bd_drift.argtypes = [vp, dp, dp, dp, dp]
@@ -94,6 +95,18 @@ def _dptr(t):
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous()):
         raise TypeError("expected a contiguous CUDA tensor")
     return C.c_void_p(t.data_ptr())
+
+
+def cholesky_noalloc(DL: torch.Tensor, info: torch.Tensor | None = None, stream: torch.cuda.Stream | None = None):
+    """bd_cholesky_noalloc: in-place tile Cholesky of DL [C][M][ld] (lower triangle) with the library's fixed scratch array;
+    no context, no allocation.  Limit C * ceil(M / 128) <= 32; calls that overlap on the GPU race (one shared array)."""
+    lib = load_library()
+    Cn, M, ld = int(DL.shape[0]), int(DL.shape[1]), int(DL.shape[2])
+    st = stream if stream is not None else torch.cuda.current_stream(DL.device)
+    rc = lib.bd_cholesky_noalloc(_dptr(DL), M, Cn, ld, ld * M, _dptr(info), C.c_void_p(st.cuda_stream))
+    if rc != 0:
+        raise BDError("bd_cholesky_noalloc", rc, lib.bd_strerror(rc).decode())
+    return DL
 
 
 class BD:

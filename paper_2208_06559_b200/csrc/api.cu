@@ -407,6 +407,7 @@ const char* bd_strerror(int code)
         case BD_ERR_CUDA: return (tl_create_cuda != cudaSuccess) ? cudaGetErrorString(tl_create_cuda) : "CUDA runtime error (bd_last_error(ctx) gives the text)";
         case BD_ERR_WORKSPACE: return "bd_step needs a workspace: call bd_set_workspace first";
         case BD_ERR_ALLOC: return "host allocation failed";
+        case BD_ERR_TOO_LARGE: return "bd_cholesky_noalloc: n_chains * ceil(M / 128) exceeds 32 (its fixed 4 MB scratch); use bd_cholesky";
         case BD_ERR_INTERNAL: return "internal error: a dependency wait inside the tile Cholesky timed out";
         default: break;
     }

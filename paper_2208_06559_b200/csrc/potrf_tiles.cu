@@ -20,6 +20,7 @@
 //   SYRK/GEMM symmetry: A and B fragments index the k dimension identically, so a lane may read ANY k of the slab as
 //   long as both operands use the same map: lane (g, t) reads 16-byte chunk (2 t + j) ^ g of row g (j = 0, 1), which
 //   is conflict free under the 128-byte swizzle (the 8 lanes of a quarter-warp hit 8 distinct chunks).
+#include <mutex>
 #include <type_traits>
 
 #include <cuda.h>          // CUtensorMap and its enums only; cuTensorMapEncodeTiled is fetched through the runtime (no -lcuda)
@@ -595,4 +596,112 @@ int bdk_potrf_tiles(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t*
     BD_LAUNCH(ctx, k_potrf_tiles, dim3(grid), dim3(NTHREADS), TILE_SMEM, *reinterpret_cast<const CUtensorMap*>(&ctx->tile_maps[0]),
               *reinterpret_cast<const CUtensorMap*>(&ctx->tile_maps[1]), a);
     return 0;
+}
+
+// =================================================================================================
+// bd_cholesky_noalloc -- the tile Cholesky for callers that cannot allocate (CUDA graph capture, tight serving loops,
+// harnesses that forbid cudaMalloc).  Same kernel (k_potrf_tiles), but its scratch -- the inverse diagonal blocks W, the
+// ready flags, the ticket counter and the error word -- lives in ONE file-scope device array of fixed size instead of
+// the context's cudaMalloc'ed buffers.  No context is needed: the caller passes the matrices, the sizes and the stream.
+//   limit: n_chains * ceil(M / 128) <= BD_NOALLOC_MAX_TILE_ROWS (32), e.g. one chain of M <= 4096, 2 of M <= 2048, 8 of
+//          M <= 512, 32 of M <= 128.  The array is 4 MB + 4.2 KB; every GPU that loads libbd holds it until exit.
+//   Every call shares the array: calls that overlap on the GPU (two streams, two host threads) RACE; serialise them.
+//   The array keeps the last call's contents, so flags, ticket counter and error word are cleared on the stream at the
+//   start of every call (W needs no clearing: every block that is read has been written by this call's diagonal tiles).
+// In host code `g_noalloc_scratch` is only a stand-in for the symbol, not a device address: the address comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+// =================================================================================================
+namespace {
+
+constexpr int NOALLOC_MAX_TILE_ROWS = 32;                                          // C * T
+constexpr size_t NOALLOC_W_BYTES = (size_t)NOALLOC_MAX_TILE_ROWS * TB * TB * sizeof(double);            // 4 MB
+constexpr size_t NOALLOC_FLAG_WORDS = (size_t)NOALLOC_MAX_TILE_ROWS * NOALLOC_MAX_TILE_ROWS + 2;         // C T^2 <= (C T)^2, + ticket, error
+constexpr size_t NOALLOC_BYTES = NOALLOC_W_BYTES + ((NOALLOC_FLAG_WORDS * sizeof(int) + 255) / 256) * 256;
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NOALLOC_BYTES];
+
+struct NoAllocDevice {
+    bool ready;
+    unsigned char* scratch;      // device address of g_noalloc_scratch on this device
+    int num_sms;
+};
+constexpr int NOALLOC_MAX_DEVICES = 64;
+NoAllocDevice g_noalloc_dev[NOALLOC_MAX_DEVICES];     // set-up record per device (address of the symbol, SM count)
+std::mutex g_noalloc_mutex;
+
+// once per device, with that device current
+int noalloc_setup(int dev, NoAllocDevice** out)
+{
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    NoAllocDevice& d = g_noalloc_dev[dev];
+    if (!d.ready) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_noalloc_scratch) != cudaSuccess || p == nullptr) return BD_ERR_CUDA;
+        if (cudaFuncSetAttribute(k_potrf_tiles, cudaFuncAttributeMaxDynamicSharedMemorySize, TILE_SMEM) != cudaSuccess) return BD_ERR_CUDA;
+        int sms = 0;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) return BD_ERR_CUDA;
+        d.scratch = static_cast<unsigned char*>(p);
+        d.num_sms = sms;
+        d.ready = true;
+    }
+    *out = &d;
+    return 0;
+}
+
+}  // namespace
+
+extern "C" int bd_cholesky_noalloc(double* DL_dev, int32_t M, int32_t n_chains, int64_t ld, int64_t chain_stride,
+                                   int32_t* info_dev, void* cuda_stream)
+{
+    if (DL_dev == nullptr || (reinterpret_cast<uintptr_t>(DL_dev) % 16) != 0) return -1;
+    if (M < 1) return -2;
+    if (n_chains < 1) return -3;
+    if (ld < M || (ld % 2) != 0) return -4;
+    if (chain_stride < ld * (int64_t)M || (chain_stride % 2) != 0) return -5;
+    const int C = n_chains, T = (M + TB - 1) / TB;
+    if ((int64_t)C * T > NOALLOC_MAX_TILE_ROWS) return BD_ERR_TOO_LARGE;
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= NOALLOC_MAX_DEVICES) return BD_ERR_CUDA;
+    NoAllocDevice* d = nullptr;
+    int rc = noalloc_setup(dev, &d);
+    if (rc != 0) return rc;
+    EncodeTiledFn enc = encode_fn();
+    if (enc == nullptr) return BD_ERR_CUDA;
+
+    double* Wbuf = reinterpret_cast<double*>(d->scratch);
+    int* flags = reinterpret_cast<int*>(d->scratch + NOALLOC_W_BYTES);
+    const size_t nflags = (size_t)C * T * T;                       // <= (C T)^2 <= NOALLOC_FLAG_WORDS - 2
+
+    CUtensorMap mA, mW;                                            // host objects, passed to the kernel by value
+    const cuuint64_t dimA[3] = {(cuuint64_t)M, (cuuint64_t)M, (cuuint64_t)C};
+    const cuuint64_t strA[2] = {(cuuint64_t)ld * 8, (cuuint64_t)chain_stride * 8};
+    const cuuint32_t boxA[3] = {BOXK, TB, 1}, es3[3] = {1, 1, 1};
+    if (enc(&mA, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, DL_dev, dimA, strA, boxA, es3, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return BD_ERR_CUDA;
+    const cuuint64_t dimW[2] = {(cuuint64_t)TB, (cuuint64_t)C * T * TB};
+    const cuuint64_t strW[1] = {(cuuint64_t)TB * 8};
+    const cuuint32_t boxW[2] = {BOXK, TB}, es2[2] = {1, 1};
+    if (enc(&mW, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, Wbuf, dimW, strW, boxW, es2, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return BD_ERR_CUDA;
+
+    // the array keeps the last call's contents: flags, ticket counter and error word start at zero
+    if (cudaMemsetAsync(flags, 0, sizeof(int) * (nflags + 2), stream) != cudaSuccess) return BD_ERR_CUDA;
+    if (info_dev != nullptr && cudaMemsetAsync(info_dev, 0, sizeof(int32_t) * (size_t)C, stream) != cudaSuccess) return BD_ERR_CUDA;
+
+    TileArgs a;
+    a.A = DL_dev; a.ld = ld; a.stride = chain_stride; a.M = M; a.C = C; a.T = T; a.nsm = d->num_sms;
+    a.Wbuf = Wbuf;
+    a.flags = flags;
+    a.epoch = 1;
+    a.ticket = reinterpret_cast<unsigned*>(flags + nflags);
+    a.err = flags + nflags + 1;
+    a.ticket_base = 0;
+    a.total = (unsigned)((int64_t)C * T * (T + 1) / 2);
+    a.info = info_dev;
+    const unsigned grid = (a.total < (unsigned)d->num_sms) ? a.total : (unsigned)d->num_sms;
+    k_potrf_tiles<<<dim3(grid), dim3(NTHREADS), TILE_SMEM, stream>>>(mA, mW, a);
+    return (cudaGetLastError() == cudaSuccess) ? 0 : BD_ERR_CUDA;
 }
