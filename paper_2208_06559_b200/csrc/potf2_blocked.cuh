@@ -82,6 +82,7 @@ __device__ __forceinline__ void gemm64(const double* __restrict__ X, const doubl
 //              then W21 = -W22 (L21 W11): two 16 x 16 x 16 products on the tensor cores (named barrier 10: W11 is ready)
 // Called from ONE place (a loop over the two halves): the fully unrolled pivot loops are ~1700 straight-line
 // instructions, and a second inlined copy ran 4x slower.
+template <bool DEFER>
 __device__ __forceinline__ void factor_half(double* __restrict__ S, double* __restrict__ Wm, double* __restrict__ sCol,
                                             double* __restrict__ sRinv, const int o, const int lane, const int warp, const int j0,
                                             int* sFail)
@@ -92,9 +93,10 @@ __device__ __forceinline__ void factor_half(double* __restrict__ S, double* __re
 #pragma unroll
         for (int j = 0; j < HB; ++j) x[j] = S[(o + max(lane, j)) * SLDP + o + min(lane, j)];
         __syncwarp();
-        const int f = warp_chol<HB, 4>(x, lane, sCol, sRinv + o, 1, [&](int k, double l) {
-            S[(o + lane) * SLDP + o + k] = (lane >= k) ? l : 0.0;
-        });
+        auto store_l = [&](int k, double l) { S[(o + lane) * SLDP + o + k] = (lane >= k) ? l : 0.0; };
+        int f;
+        if constexpr (DEFER) f = warp_chol_deferred<HB, 4>(x, lane, sCol, sRinv + o, 1, store_l);
+        else f = warp_chol<HB, 4>(x, lane, sCol, sRinv + o, 1, store_l);
         if (lane == 0 && f != 0 && *sFail == 0) *sFail = j0 + o + f;
     } else if (warp == 1) {
         warp_inverse_f<QB, 4>(lane, QB, sRinv + o, 1, [&](int k, int j) { return S[(o + k) * SLDP + o + j]; },
@@ -155,7 +157,7 @@ __device__ __forceinline__ void factor_half(double* __restrict__ S, double* __re
 // ONE copy of the factor / inverse code, run once per half: a second inlined copy (64 KB further into the kernel) ran 4x
 // slower than the first one (22 k against 5.5 k cycles for the same 32 pivots -- instruction fetch of ~1700 straight-line
 // instructions that are cold at every launch), a loop re-runs warm instructions.
-template <class Sync>
+template <bool DEFER = false, class Sync>
 __device__ __forceinline__ void block64(double* __restrict__ S, double* __restrict__ Wm, double* __restrict__ sCol,
                                         double* __restrict__ sRinv, const int nh, const int lane, const int warp, const int row0,
                                         int* sFail, Sync&& sync)
@@ -164,7 +166,7 @@ __device__ __forceinline__ void block64(double* __restrict__ S, double* __restri
     double out[2][2];
 #pragma unroll 1
     for (int hh = 0; hh < nh; ++hh) {
-        factor_half(S, Wm, sCol, sRinv, hh * HB, lane, warp, row0, sFail);
+        factor_half<DEFER>(S, Wm, sCol, sRinv, hh * HB, lane, warp, row0, sFail);
         sync();
         if (hh == 0 && nh == 2) {
             gemm32(S + HB * SLDP, Wm, false, warp, lane, out);         // L21 = A21 W11^T

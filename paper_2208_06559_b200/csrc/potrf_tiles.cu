@@ -171,6 +171,9 @@ __device__ __forceinline__ void trsm_box(double (&acc)[4][8][2], const int wn, c
     }
 }
 
+// LATENCY = true: the instance for factorisations with few tiles per column (one chain of moderate size), where the
+// diagonal tiles are the critical path: its factoring warp defers the rank-1 update (warp_chol_deferred).
+template <bool LATENCY>
 __global__ void __launch_bounds__(NTHREADS, 1) k_potrf_tiles(const __grid_constant__ CUtensorMap tmA,
                                                              const __grid_constant__ CUtensorMap tmW, const TileArgs a)
 {
@@ -443,7 +446,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_potrf_tiles(const __grid_consta
                 double* Sb = hh ? S22 : S11;
                 double* Wb = hh ? W22 : W11;
                 const int nrem = nloc - 64 * hh;
-                potf2::block64(Sb, Wb, sCol, sRinv, (nrem > potf2::HB) ? 2 : 1, lane, warp, tn0 + 64 * hh, &sFail, [] { cons_sync(); });
+                potf2::block64<LATENCY>(Sb, Wb, sCol, sRinv, (nrem > potf2::HB) ? 2 : 1, lane, warp, tn0 + 64 * hh, &sFail, [] { cons_sync(); });
                 if (hh == 0) {
                     potf2::gemm64(S21, W11, false, warp, lane, o);             // L21 = S21 W11^T
                     cons_sync();
@@ -559,7 +562,8 @@ int bdk_potrf_tiles(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t*
         ctx->tile_flags = flags;
         ctx->tile_epoch = 0;
         ctx->tile_ticket_base = 0;
-        BD_CUDA(ctx, cudaFuncSetAttribute(k_potrf_tiles, cudaFuncAttributeMaxDynamicSharedMemorySize, TILE_SMEM));
+        BD_CUDA(ctx, cudaFuncSetAttribute(k_potrf_tiles<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TILE_SMEM));
+        BD_CUDA(ctx, cudaFuncSetAttribute(k_potrf_tiles<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TILE_SMEM));
     }
     EncodeTiledFn enc = encode_fn();
     if (enc == nullptr) { ctx->last_cuda = cudaErrorNotSupported; return BD_ERR_CUDA; }
@@ -593,8 +597,13 @@ int bdk_potrf_tiles(bd_ctx* ctx, double* A, int64_t ld, int64_t stride, int32_t*
     a.info = info;
     const unsigned grid = (a.total < (unsigned)ctx->num_sms) ? a.total : (unsigned)ctx->num_sms;
     ctx->tile_ticket_base += a.total + grid;          // every CTA's producer draws exactly one ticket beyond the last tile
-    BD_LAUNCH(ctx, k_potrf_tiles, dim3(grid), dim3(NTHREADS), TILE_SMEM, *reinterpret_cast<const CUtensorMap*>(&ctx->tile_maps[0]),
-              *reinterpret_cast<const CUtensorMap*>(&ctx->tile_maps[1]), a);
+    const CUtensorMap& mapA = *reinterpret_cast<const CUtensorMap*>(&ctx->tile_maps[0]);
+    const CUtensorMap& mapW = *reinterpret_cast<const CUtensorMap*>(&ctx->tile_maps[1]);
+    // few tiles per column (C T / 2 on average, against num_sms CTAs): the diagonal tiles are the critical path
+    if ((int64_t)C * T <= 2 * ctx->num_sms && T <= 64)
+        BD_LAUNCH(ctx, k_potrf_tiles<true>, dim3(grid), dim3(NTHREADS), TILE_SMEM, mapA, mapW, a);
+    else
+        BD_LAUNCH(ctx, k_potrf_tiles<false>, dim3(grid), dim3(NTHREADS), TILE_SMEM, mapA, mapW, a);
     return 0;
 }
 
@@ -637,7 +646,7 @@ int noalloc_setup(int dev, NoAllocDevice** out)
     if (!d.ready) {
         void* p = nullptr;
         if (cudaGetSymbolAddress(&p, g_noalloc_scratch) != cudaSuccess || p == nullptr) return BD_ERR_CUDA;
-        if (cudaFuncSetAttribute(k_potrf_tiles, cudaFuncAttributeMaxDynamicSharedMemorySize, TILE_SMEM) != cudaSuccess) return BD_ERR_CUDA;
+        if (cudaFuncSetAttribute(k_potrf_tiles<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TILE_SMEM) != cudaSuccess) return BD_ERR_CUDA;
         int sms = 0;
         if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) return BD_ERR_CUDA;
         d.scratch = static_cast<unsigned char*>(p);
@@ -702,6 +711,6 @@ extern "C" int bd_cholesky_noalloc(double* DL_dev, int32_t M, int32_t n_chains, 
     a.total = (unsigned)((int64_t)C * T * (T + 1) / 2);
     a.info = info_dev;
     const unsigned grid = (a.total < (unsigned)d->num_sms) ? a.total : (unsigned)d->num_sms;
-    k_potrf_tiles<<<dim3(grid), dim3(NTHREADS), TILE_SMEM, stream>>>(mA, mW, a);
+    k_potrf_tiles<false><<<dim3(grid), dim3(NTHREADS), TILE_SMEM, stream>>>(mA, mW, a);
     return (cudaGetLastError() == cudaSuccess) ? 0 : BD_ERR_CUDA;
 }

@@ -81,6 +81,70 @@ __device__ __forceinline__ int warp_chol(double (&x)[NB], const int lane, double
     return fail;
 }
 
+// The same elimination with the rank-1 update DEFERRED by one pivot.  One warp issues in order, so in warp_chol every
+// update FMA that follows the LDS of the column just broadcast stalls the whole warp, chain included (measured: 390
+// cycles per pivot for a dependent chain of ~130: MUFU.RSQ64H, 10 FP64 ops, SHFL).  Here pivot k
+//   - applies pivot k-1 to the columns j >= k+1 from REGISTERS (cp[], loaded one pivot ago: the data has arrived),
+//   - takes the one value the chain needs now, l_{k+1,k}, by shuffle and updates column k+1 with it at once,
+//   - issues the loads of column k (j >= k+2) for the next pivot.
+// Costs NB more registers (cp[]); inside the tile kernel that pressure makes ptxas spill in the DMMA loops, so it is used
+// only by the kernel instance for latency-bound factorisations (few tiles per column: the diagonal tiles are the
+// critical path and the DMMA loops are not the limiter).
+template <int NB, int CH, class StoreL>
+__device__ __forceinline__ int warp_chol_deferred(double (&x)[NB], const int lane, double* __restrict__ s_col,
+                                                  double* __restrict__ s_rinv, const int bar0, StoreL&& store_l)
+{
+    static_assert(NB <= 32 && (NB % 2) == 0 && (NB % CH) == 0, "warp_chol_deferred: NB even, <= 32, multiple of CH");
+    int fail = 0;
+    double d = __shfl_sync(0xffffffffu, x[0], 0);
+    double lm_prev = 0.0;                     // this lane's l of pivot k-1 (0 for lanes <= k-1)
+    double cp[NB];                            // column k-1 of L (cp[j] = l_{j,k-1}), valid for j >= k+1
+#pragma unroll
+    for (int j = 0; j < NB; ++j) cp[j] = 0.0;
+#pragma unroll
+    for (int k = 0; k < NB; ++k) {
+        if (!(d > 0.0) && fail == 0) fail = k + 1;
+        const double rinv = fast_rsqrt_pos(d);
+        const double l = x[k] * rinv;          // x[k] carries every pivot < k (pivot k-1 was applied eagerly below)
+        if (k >= 1) {
+#pragma unroll
+            for (int j = k + 1; j < NB; ++j) x[j] = fma(-lm_prev, cp[j], x[j]);      // pivot k-1, deferred
+        }
+        if (k + 1 < NB) {
+            const double dn = fma(-l, l, x[k + 1 < NB ? k + 1 : k]);
+            d = __shfl_sync(0xffffffffu, dn, k + 1);
+        }
+        store_l(k, l);
+        if (lane == k) s_rinv[k] = rinv;
+        const double lm = (lane > k) ? l : 0.0;
+        double* col = s_col + (k & 1) * 32;
+        col[lane] = lm;
+        __syncwarp();
+        if (k + 1 < NB) {
+            const double lk1 = __shfl_sync(0xffffffffu, lm, k + 1);                 // l_{k+1,k}: column k+1 is needed next
+            x[k + 1 < NB ? k + 1 : k] = fma(-lm, lk1, x[k + 1 < NB ? k + 1 : k]);
+        }
+        // column k for the next pivot's deferred update (j >= k+2), 16-byte loads where the pair is aligned
+        if ((k & 1) == 0) {
+#pragma unroll
+            for (int j = k + 2; j + 1 < NB; j += 2) {
+                const double2 c2 = *reinterpret_cast<const double2*>(col + j);
+                cp[j] = c2.x; cp[j + 1] = c2.y;
+            }
+        } else {
+            if (k + 2 < NB) cp[k + 2 < NB ? k + 2 : k] = col[k + 2 < NB ? k + 2 : k];
+#pragma unroll
+            for (int j = k + 3; j + 1 < NB; j += 2) {
+                const double2 c2 = *reinterpret_cast<const double2*>(col + j);
+                cp[j] = c2.x; cp[j + 1] = c2.y;
+            }
+        }
+        lm_prev = lm;
+        if ((k + 1) % CH == 0) named_arrive(bar0 + k / CH, 64);
+    }
+    return fail;
+}
+
 // Inverse factor by forward substitution, lane c = column c of W = L^-1 (lower):
 //     W[k][c] = (delta_kc - sum_{j<k} L[k][j] W[j][c]) / L[k][k]
 // L(k, j) (j < k) and s_rinv[k] come from shared memory as broadcast loads once the factoring warp has arrived on the
