@@ -53,6 +53,16 @@ def test_no_cpu_fallback_without_a_gpu():
     assert lib.bd_create(C.byref(p), None, C.byref(ctx)) == binding.ERR_CUDA
     assert ctx.value is None
     assert lib.bd_step(None, None, 0, 1) == -1
+    # the context-free entry point validates its arguments before touching the device
+    assert lib.bd_cholesky_noalloc(None, 10, 1, 10, 100, None, None) == -1
+    buf = C.create_string_buffer(64)
+    addr = (C.addressof(buf) + 15) // 16 * 16
+    assert lib.bd_cholesky_noalloc(C.c_void_p(addr), 0, 1, 10, 100, None, None) == -2
+    assert lib.bd_cholesky_noalloc(C.c_void_p(addr), 10, 0, 10, 100, None, None) == -3
+    assert lib.bd_cholesky_noalloc(C.c_void_p(addr), 10, 1, 9, 100, None, None) == -4
+    assert lib.bd_cholesky_noalloc(C.c_void_p(addr), 10, 1, 10, 99, None, None) == -5
+    assert lib.bd_cholesky_noalloc(C.c_void_p(addr), 128, 33, 128, 128 * 128, None, None) == binding.ERR_TOO_LARGE
+    assert b"32" in lib.bd_strerror(binding.ERR_TOO_LARGE)
 
 
 def test_product_does_not_import_the_oracle():
