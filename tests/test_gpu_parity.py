@@ -420,3 +420,14 @@ def test_relaxation_time_pipeline_free_draining():
     row = relaxation.measure(10, 2048, 0.0, 1e-3, 2.0, 50)
     assert 0.9 < row["lambda"] / row["lambda_rouse"] < 1.7
     assert abs(row["Ree"] ** 2 / 10.0 - 1.0) < 0.1                                # <R^2> = N b^2 at equilibrium
+
+
+def test_relaxation_run_resumed_from_a_checkpoint_is_the_uninterrupted_run(tmp_path):
+    """relaxation.measure with a time budget of zero stops after one sample and writes its state; resumed, it returns
+    exactly the row of the uninterrupted run (counter-based noise, deterministic kernels)."""
+    from paper_2208_06559_b200 import relaxation
+    full = relaxation.measure(10, 256, 0.25, 1e-3, 1.0, 20)
+    ck = str(tmp_path / "ck.npz")
+    assert relaxation.measure(10, 256, 0.25, 1e-3, 1.0, 20, save=ck, budget_s=0.0) is None
+    cont = relaxation.measure(10, 256, 0.25, 1e-3, 1.0, 20, resume=ck)
+    assert cont == full
